@@ -1,0 +1,327 @@
+// arkcos_api.cu - the C ABI of include/arkcos.h: plan creation (S1 + uploads), the hot-path launches
+// (S2 weight generator, S3 convolution) and the introspection / measurement hooks.
+// Product code; shares nothing with oracle/.  No CPU fallback: compute entry points need a CUDA device.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/arkcos.h"
+#include "arkcos_internal.h"
+#include "arkcos_kernels.cuh"
+
+using namespace arkcos;
+
+namespace {
+thread_local std::string g_last_cuda_error;
+
+bool cuda_ok(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+    (void)cudaGetLastError();
+    return false;
+}
+#define CU(call) do { if (!cuda_ok((call), #call)) return ARKCOS_ECUDA; } while (0)
+}  // namespace
+
+struct arkcos_plan {
+    Schedule sched;
+    std::vector<double> table;
+    int n_table = 0;
+    unsigned flags = 0;
+    int device = -1, sm_count = 0;
+    bool weights_ready = false;       // cached plans: generator already ran
+    // device memory
+    PairDesc* d_pairs = nullptr;
+    Item* d_items = nullptr;
+    GenUnit* d_units = nullptr;
+    double *d_sin_t = nullptr, *d_area = nullptr, *d_a_r = nullptr, *d_s2 = nullptr, *d_table = nullptr;
+    float* d_weights = nullptr;
+    float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging, lazily allocated
+    size_t device_bytes = 0;
+    size_t conv_smem = 0, gen_smem = 0;
+    int gen_grid = 0, table_in_smem = 0;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+};
+
+namespace {
+
+template <typename T>
+arkcos_status upload(arkcos_plan* pl, T** dst, const std::vector<T>& src) {
+    size_t bytes = src.size() * sizeof(T);
+    if (bytes == 0) bytes = sizeof(T);
+    cudaError_t e = cudaMalloc((void**)dst, bytes);
+    if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); return ARKCOS_ENOMEM; }
+    CU(e);
+    pl->device_bytes += bytes;
+    if (!src.empty()) CU(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return ARKCOS_OK;
+}
+
+arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
+    GenParams g;
+    g.pairs = pl->d_pairs; g.units = pl->d_units; g.sin_t = pl->d_sin_t; g.area = pl->d_area;
+    g.a_r = pl->d_a_r; g.s2 = pl->d_s2; g.table = pl->d_table; g.weights = pl->d_weights;
+    g.n_units = (int)pl->sched.gen_units.size(); g.n_theta = pl->sched.n_theta; g.n_phi = pl->sched.n_phi;
+    g.n_table = pl->n_table; g.R = pl->sched.R;
+    g.t_scale = (double)(pl->n_table - 1) / pl->sched.theta_cut;
+    g.table_in_smem = pl->table_in_smem;
+    k_generate_weights<<<pl->gen_grid, 256, pl->gen_smem, st>>>(g);
+    CU(cudaGetLastError());
+    return ARKCOS_OK;
+}
+
+arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
+    ConvParams c;
+    c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
+    c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R;
+    c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
+    dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
+    k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
+    CU(cudaGetLastError());
+    return ARKCOS_OK;
+}
+
+arkcos_status check_io(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps) {
+    if (!pl || !d_in || !d_out || n_maps < 1) return ARKCOS_EINVAL;
+    if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    if (((uintptr_t)d_in & 15u) || ((uintptr_t)d_out & 15u)) return ARKCOS_EINVAL;
+    const size_t bytes = (size_t)n_maps * pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
+    const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+    if (a < b + bytes && b < a + bytes) return ARKCOS_EINVAL;   // overlap
+    return ARKCOS_OK;
+}
+
+arkcos_status run(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
+    const bool cached = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) != 0;
+    if (!cached) { arkcos_status s = launch_generate(pl, st); if (s != ARKCOS_OK) return s; }
+    return launch_convolve(pl, d_in, d_out, n_maps, st);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* arkcos_status_string(arkcos_status s) {
+    switch (s) {
+        case ARKCOS_OK: return "ARKCOS_OK";
+        case ARKCOS_EINVAL: return "ARKCOS_EINVAL: invalid argument";
+        case ARKCOS_ENOMEM: return "ARKCOS_ENOMEM: out of memory";
+        case ARKCOS_ECUDA: return "ARKCOS_ECUDA: CUDA runtime error";
+        case ARKCOS_EUNSUPPORTED: return "ARKCOS_EUNSUPPORTED: not supported by this build";
+    }
+    return "ARKCOS_?: unknown status";
+}
+
+const char* arkcos_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
+    if (!pl) return ARKCOS_OK;
+    if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
+        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_sin_t);
+        cudaFree(pl->d_area); cudaFree(pl->d_a_r); cudaFree(pl->d_s2); cudaFree(pl->d_table);
+        cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
+        for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
+        (void)cudaGetLastError();
+    }
+    delete pl;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, const double* k_table, int n_table,
+                                    double theta_cut, unsigned flags) {
+    if (!plan) return ARKCOS_EINVAL;
+    *plan = nullptr;
+    if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
+    if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS)) return ARKCOS_EINVAL;
+    for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
+    arkcos_plan* pl = new (std::nothrow) arkcos_plan();
+    if (!pl) return ARKCOS_ENOMEM;
+    pl->flags = flags; pl->n_table = n_table;
+    arkcos_status st = ARKCOS_OK;
+    try {
+        pl->table.assign(k_table, k_table + n_table);
+        if (!(flags & ARKCOS_PLAN_HOST_ONLY)) {
+            cudaDeviceProp prop;
+            if (!cuda_ok(cudaGetDevice(&pl->device), "cudaGetDevice") ||
+                !cuda_ok(cudaGetDeviceProperties(&prop, pl->device), "cudaGetDeviceProperties")) {
+                delete pl; return ARKCOS_ECUDA;
+            }
+            pl->sm_count = prop.multiProcessorCount;
+            if (prop.major < 10) { g_last_cuda_error = "arkcos needs an sm_100 class device"; delete pl; return ARKCOS_EUNSUPPORTED; }
+        }
+        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
+        if (rc != 0) { delete pl; return (arkcos_status)rc; }
+    } catch (const std::bad_alloc&) { delete pl; return ARKCOS_ENOMEM; }
+    if (flags & ARKCOS_PLAN_HOST_ONLY) { *plan = pl; return ARKCOS_OK; }
+
+    const Schedule& s = pl->sched;
+    do {
+        if ((st = upload(pl, &pl->d_pairs, s.pairs)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_items, s.items)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_units, s.gen_units)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_sin_t, s.sin_t)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_area, s.area)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_a_r, s.a_r)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_s2, s.s2)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_table, pl->table)) != ARKCOS_OK) break;
+        {
+            size_t bytes = (size_t)s.weight_slots * sizeof(float) + 16;
+            cudaError_t e = cudaMalloc((void**)&pl->d_weights, bytes);
+            if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); st = ARKCOS_ENOMEM; break; }
+            if (!cuda_ok(e, "cudaMalloc(weights)")) { st = ARKCOS_ECUDA; break; }
+            pl->device_bytes += bytes;
+        }
+        // launch configuration
+        int f_max = 0;
+        for (const Item& it : s.items) f_max = it.f_log2 > f_max ? it.f_log2 : f_max;
+        size_t smem = 0;
+        for (int fl = 0; fl <= f_max; fl++) { size_t b = conv_smem_bytes(fl); smem = b > smem ? b : smem; }
+        pl->conv_smem = smem;
+        if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                     "cudaFuncSetAttribute(k_convolve)")) { st = ARKCOS_ECUDA; break; }
+        size_t tab_bytes = (size_t)n_table * sizeof(double);
+        pl->table_in_smem = tab_bytes <= 200 * 1024 ? 1 : 0;
+        pl->gen_smem = pl->table_in_smem ? tab_bytes : 0;
+        if (!cuda_ok(cudaFuncSetAttribute(k_generate_weights, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(pl->gen_smem > 0 ? pl->gen_smem : 1)),
+                     "cudaFuncSetAttribute(k_generate_weights)")) { st = ARKCOS_ECUDA; break; }
+        int units = (int)s.gen_units.size();
+        pl->gen_grid = units < pl->sm_count ? (units > 0 ? units : 1) : pl->sm_count;
+        for (auto& e : pl->ev)
+            if (!cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) { st = ARKCOS_ECUDA; break; }
+        if (st != ARKCOS_OK) break;
+        if (flags & ARKCOS_PLAN_CACHE_WEIGHTS) {
+            if ((st = launch_generate(pl, 0)) != ARKCOS_OK) break;
+            if (!cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) { st = ARKCOS_ECUDA; break; }
+            pl->weights_ready = true;
+        }
+    } while (0);
+    if (st != ARKCOS_OK) { arkcos_plan_destroy(pl); return st; }
+    *plan = pl;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_create(arkcos_plan** plan, int n_theta, int n_phi, const double* k_table, int n_table,
+                                 double theta_cut) {
+    return arkcos_plan_create_ex(plan, n_theta, n_phi, k_table, n_table, theta_cut, ARKCOS_PLAN_DEFAULT);
+}
+
+arkcos_status arkcos_convolve_batch(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, void* stream) {
+    arkcos_status s = check_io(pl, d_in, d_out, n_maps);
+    if (s != ARKCOS_OK) return s;
+    if (n_maps > 65535) return ARKCOS_EINVAL;
+    return run(pl, d_in, d_out, n_maps, (cudaStream_t)stream);
+}
+
+arkcos_status arkcos_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, void* stream) {
+    return arkcos_convolve_batch(pl, d_in, d_out, 1, stream);
+}
+
+arkcos_status arkcos_convolve_timed(const arkcos_plan* pl, const float* d_in, float* d_out, void* stream,
+                                    float* ms_generate, float* ms_convolve) {
+    arkcos_status s = check_io(pl, d_in, d_out, 1);
+    if (s != ARKCOS_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool cached = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) != 0;
+    CU(cudaEventRecord(pl->ev[0], st));
+    if (!cached) { if ((s = launch_generate(pl, st)) != ARKCOS_OK) return s; }
+    CU(cudaEventRecord(pl->ev[1], st));
+    if ((s = launch_convolve(pl, d_in, d_out, 1, st)) != ARKCOS_OK) return s;
+    CU(cudaEventRecord(pl->ev[2], st));
+    CU(cudaEventSynchronize(pl->ev[2]));
+    float a = 0.f, b = 0.f;
+    CU(cudaEventElapsedTime(&a, pl->ev[0], pl->ev[1]));
+    CU(cudaEventElapsedTime(&b, pl->ev[1], pl->ev[2]));
+    if (ms_generate) *ms_generate = cached ? 0.f : a;
+    if (ms_convolve) *ms_convolve = b;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_convolve_host(arkcos_plan* pl, const float* h_in, float* h_out, void* stream) {
+    if (!pl || !h_in || !h_out) return ARKCOS_EINVAL;
+    if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
+    if (!pl->d_io_in) {
+        cudaError_t e = cudaMalloc((void**)&pl->d_io_in, bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d_io_out, bytes);
+        if (e == cudaErrorMemoryAllocation) {
+            (void)cudaGetLastError(); cudaFree(pl->d_io_in); pl->d_io_in = nullptr; return ARKCOS_ENOMEM;
+        }
+        CU(e);
+        pl->device_bytes += 2 * bytes;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemcpyAsync(pl->d_io_in, h_in, bytes, cudaMemcpyHostToDevice, st));
+    arkcos_status s = run(pl, pl->d_io_in, pl->d_io_out, 1, st);
+    if (s != ARKCOS_OK) return s;
+    CU(cudaMemcpyAsync(h_out, pl->d_io_out, bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_work(const arkcos_plan* pl, unsigned long long* pair_evals, unsigned long long* weights,
+                               int* ring_halfband) {
+    if (!pl) return ARKCOS_EINVAL;
+    if (pair_evals) *pair_evals = pl->sched.pair_evals;
+    if (weights) *weights = pl->sched.weights;
+    if (ring_halfband) *ring_halfband = pl->sched.R;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_get_info(const arkcos_plan* pl, arkcos_plan_info* info) {
+    if (!pl || !info) return ARKCOS_EINVAL;
+    std::memset(info, 0, sizeof(*info));
+    const Schedule& s = pl->sched;
+    info->n_theta = s.n_theta; info->n_phi = s.n_phi; info->n_table = pl->n_table; info->theta_cut = s.theta_cut;
+    info->ring_halfband = s.R; info->pair_evals = s.pair_evals; info->weights = s.weights;
+    info->fma_slots = s.fma_slots; info->weight_slots = s.weight_slots;
+    info->n_items = (int)s.items.size(); info->n_gen_units = (int)s.gen_units.size();
+    info->kernels_per_convolve = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) ? 1 : 2;
+    info->sm_count = pl->sm_count; info->flags = pl->flags; info->device_bytes = pl->device_bytes;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_window(const arkcos_plan* pl, int i, int j, int* half_width) {
+    if (!pl || !half_width) return ARKCOS_EINVAL;
+    if (i < 0 || i >= pl->sched.n_theta || j < 0 || j >= pl->sched.n_theta) return ARKCOS_EINVAL;
+    *half_width = pl->sched.window(i, j);
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_pair_weights(const arkcos_plan* pl, int i, int j, float* h_w, int cap, int* n) {
+    if (!pl || !h_w || !n || cap < 0) return ARKCOS_EINVAL;
+    if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    const Schedule& s = pl->sched;
+    if (i < 0 || i >= s.n_theta || j < 0 || j >= s.n_theta) return ARKCOS_EINVAL;
+    *n = 0;
+    // southern output rings use their northern mirror pair (identical weights)
+    int in_ = i, jn = j;
+    if (i >= s.n_north) { in_ = s.n_theta - 1 - i; jn = s.n_theta - 1 - j; }
+    const PairDesc* pd = s.pair(in_, jn);
+    if (!pd || pd->ntaps == 0) return ARKCOS_OK;
+    if (!pl->weights_ready) {
+        arkcos_status st = launch_generate(pl, 0);
+        if (st != ARKCOS_OK) return st;
+    }
+    CU(cudaDeviceSynchronize());
+    int dmax = pd->half == s.n_phi ? s.n_phi / 2 : pd->half;
+    int cnt = dmax + 1 < cap ? dmax + 1 : cap;
+    std::vector<float> all(pd->ntaps);
+    CU(cudaMemcpy(all.data(), pl->d_weights + pd->w_off, sizeof(float) * pd->ntaps, cudaMemcpyDeviceToHost));
+    for (int d = 0; d < cnt; d++) {
+        // tap +d is stored at e = d - start, except d = n_phi/2 of a whole ring, stored as d = -n_phi/2 (e = 0)
+        int e = d - pd->start;
+        if (e >= pd->ntaps) e = 0;
+        h_w[d] = all[e];
+    }
+    *n = cnt;
+    return ARKCOS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,139 @@
+// arkcos_schedule.cpp - step S1, the ring-pair scheduler (host, FP64).  BASELINE.json north_star (a):
+// "a ring-pair scheduler that exploits the ECP grid's azimuthal symmetry, so each (output ring i,
+// input ring j) pair inside the theta_cut band is a banded circular 1-D convolution in dphi".
+// SURVEY.md §8(a)-S1, §8(c) G3 (support decided in FP64), G12 (poles / whole-ring windows).
+//
+// Geometry uses the cancellation-free haversine form, algebraically identical to
+// cos(gamma) = cos t_i cos t_j + sin t_i sin t_j cos(dphi):
+//     sin^2(gamma/2) = sin^2((t_i - t_j)/2) + sin t_i sin t_j sin^2(dphi/2)
+// and the support test  gamma <= theta_cut  <=>  sin^2(gamma/2) <= sin^2(theta_cut/2).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+
+#include "arkcos_internal.h"
+
+namespace arkcos {
+
+namespace {
+constexpr double kPi = 3.14159265358979323846264338327950288;
+
+// The single FP64 expression that decides whether tap d of ring pair (a_r, b) is inside the support.
+inline bool inside(const Schedule& s, double a_r, double b, int d) { return a_r + b * s.s2[d] <= s.h_cut; }
+
+// -1 empty, n_phi whole ring, else largest D with tap D inside (monotone in d on [0, n_phi/2]).
+int window_of(const Schedule& s, int i, int j) {
+    int r = std::abs(i - j);
+    if (r > s.R) return -1;
+    double a_r = s.a_r[r];
+    double b = s.sin_t[i] * s.sin_t[j];
+    if (!inside(s, a_r, b, 0)) return -1;
+    int half = s.n_phi / 2;
+    if (inside(s, a_r, b, half)) return s.n_phi;
+    int lo = 0, hi = half;  // inside(lo) true, inside(hi) false
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (inside(s, a_r, b, mid)) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+}  // namespace
+
+int Schedule::window(int i, int j) const {
+    if (i < 0 || i >= n_theta || j < 0 || j >= n_theta) return -1;
+    return window_of(*this, i, j);
+}
+
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s) {
+    if (n_theta < 1 || n_phi < 4 || !(theta_cut > 0.0) || !(theta_cut <= kPi * (1.0 + 1e-15))) return 1;
+    if (n_phi % 4 != 0) return 4;
+    if (sm_count < 1) sm_count = 148;
+    s = Schedule();
+    s.n_theta = n_theta; s.n_phi = n_phi; s.theta_cut = theta_cut;
+    s.n_north = (n_theta + 1) / 2;
+    const double dtheta = kPi / n_theta, dphi = 2.0 * kPi / n_phi;
+    {
+        double sh = std::sin(0.5 * std::min(theta_cut, kPi));
+        s.h_cut = sh * sh;
+    }
+    s.sin_t.resize(n_theta); s.area.resize(n_theta);
+    for (int i = 0; i < n_theta; i++) {
+        s.sin_t[i] = std::sin((i + 0.5) * dtheta);
+        // exact ring pixel area dphi (cos(j dt) - cos((j+1) dt)) in its product form (no cancellation)
+        s.area[i] = 2.0 * dphi * s.sin_t[i] * std::sin(0.5 * dtheta);
+    }
+    s.s2.resize(n_phi / 2 + 1);
+    for (int d = 0; d <= n_phi / 2; d++) { double v = std::sin(0.5 * d * dphi); s.s2[d] = v * v; }
+    // ring half band R: largest r whose d = 0 tap is inside (gamma >= |t_i - t_j|, equality at d = 0)
+    s.a_r.clear();
+    for (int r = 0; r < n_theta; r++) {
+        double v = std::sin(0.5 * r * dtheta); v *= v;
+        if (v > s.h_cut) break;
+        s.a_r.push_back(v);
+    }
+    s.R = (int)s.a_r.size() - 1;
+    const int W = 2 * s.R + 1;
+
+    // ---- pair descriptors for the northern rings; work counters over ALL rings ------------------
+    s.pairs.assign((size_t)s.n_north * W, PairDesc{0u, 0, 0, -1});
+    unsigned long long w_off = 0;
+    std::vector<unsigned long long> ring_slots(s.n_north, 0);  // stored taps per output phi
+    for (int i = 0; i < n_theta; i++) {
+        for (int r = -s.R; r <= s.R; r++) {
+            int j = i + r;
+            if (j < 0 || j >= n_theta) continue;            // no wrap over the pole (G12)
+            int D = window_of(s, i, j);
+            if (D < 0) continue;
+            unsigned long long taps = (D == n_phi) ? (unsigned long long)n_phi : (unsigned long long)(2 * D + 1);
+            s.weights += taps;
+            s.pair_evals += taps * (unsigned long long)n_phi;
+            if (i < s.n_north) {
+                PairDesc& p = s.pairs[(size_t)i * W + (r + s.R)];
+                p.half = D;
+                if (D == n_phi) { p.start = -(n_phi / 2); p.ntaps = n_phi; }
+                else { p.start = -(D + (D & 1)); p.ntaps = ((D - p.start + 1) + 3) & ~3; }
+                if (w_off + (unsigned long long)p.ntaps > 0xFFFFFFF0ull) return 4;
+                p.w_off = (uint32_t)w_off;
+                w_off += (unsigned long long)p.ntaps;
+                ring_slots[i] += (unsigned long long)p.ntaps;
+            }
+        }
+    }
+    s.weight_slots = w_off;
+
+    // ---- generator work units -------------------------------------------------------------------
+    for (size_t pi = 0; pi < s.pairs.size(); pi++)
+        for (int e0 = 0; e0 < s.pairs[pi].ntaps; e0 += kGenUnitTaps) s.gen_units.push_back(GenUnit{(uint32_t)pi, (uint32_t)e0});
+
+    // ---- work items: (north ring, phi tile), tile width 512 F chosen so that no item exceeds
+    //      ~1/6 of one SM's share of the whole job; heaviest first (H1: polar imbalance) ------------
+    unsigned long long total = 0;
+    for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi;
+    double c_max = (double)total / (double)sm_count / 6.0;
+    struct Tmp { Item it; double cost; };
+    std::vector<Tmp> tmp;
+    int f_cap = 0;                                            // largest useful F for this n_phi
+    while (f_cap < 3 && (kWarpSpan << f_cap) < n_phi) f_cap++;
+    for (int i = 0; i < s.n_north; i++) {
+        if (ring_slots[i] == 0) {
+            // ring with no work still needs its output zeroed: one cheap item per tile
+        }
+        int fl = f_cap;
+        while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWarpSpan << fl) > c_max) fl--;
+        int L = kWarpSpan << fl;
+        for (int k0 = 0; k0 < n_phi; k0 += L) {
+            int span = std::min(L, n_phi - k0);
+            double cost = (double)ring_slots[i] * (double)L + 2000.0;   // issued slots, not useful ones
+            tmp.push_back(Tmp{Item{i, k0, fl, 0}, cost});
+            // both mirror rings: 2 FMA lanes per slot (one FFMA2)
+            s.fma_slots += 2ull * ring_slots[i] * (unsigned long long)L;
+            (void)span;
+        }
+    }
+    std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
+    s.items.reserve(tmp.size());
+    for (auto& t : tmp) s.items.push_back(t.it);
+    return 0;
+}
+
+}  // namespace arkcos
