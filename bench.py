@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the real-space spherical convolution hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+    torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N --steps K --warmup W
+
+One "step" = one pass of the whole hot path (S2 weight generator + S3 convolution, all rows of
+SURVEY.md §8(a); S1 is plan-time) over one synthetic map of the workload.  Default workload:
+BASELINE.json configs[2], the Planck-resolution case north_star's target is quoted on.
+Prints ONE JSON line (rank 0).  `--sweep` prints the five-config report and the cost-vs-theta_cut
+curve instead (one JSON line per workload, then a fit line).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1211_3556_b200 import replicas  # noqa: E402
+from paper_1211_3556_b200 import workloads as wl  # noqa: E402
+
+METRIC = "kernel-pixel evaluations/s at theta_cut (output pixels/s alongside)"
+UNIT = "kernel-pixel evals/s"
+DEFAULT_WORKLOAD = "cfg2_planck_4096x8192_fwhm5"
+# FP32 FMA roofline of one B200: SMs x 128 FP32 lanes x 2 flop x max SM clock (B200_PROFILING.md:
+# 148 SMs, clocks.max.sm 1965 MHz; 128 FP32 lanes per SM, 4 SMSPs x 32).  DESIGN.md §Roofline.
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+def ncu_traffic(workload: str):
+    """dram bytes per launch of the convolution kernel from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        parts = [p.strip() for p in line.split(",")]
+        if len(parts) >= 3 and parts[0] == workload and parts[1] == "k_convolve":
+            try:
+                return float(parts[2])
+            except ValueError:
+                return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="arkcos_clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        try:
+            sm, mx, reasons, pw = [], [], set(), []
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1])); mx.append(float(p[2])); pw.append(float(p[3]))
+                except ValueError:
+                    continue
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            if sm:
+                out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                       "samples": len(sm), "power_w_max": float(max(pw))}
+        except Exception:
+            pass
+        finally:
+            try:
+                os.unlink(self.path)
+            except Exception:
+                pass
+        return out
+
+
+def oracle_sample(w: wl.Workload, n_pixels: int, seed: int):
+    """Time the CPU oracle, as it stands, on a seeded uniform sample of output pixels of `w`."""
+    from oracle import oracle
+    rng = np.random.default_rng(seed)
+    pix = rng.integers(0, w.n_pix, size=n_pixels).astype(np.int64)
+    x = w.map_f32()
+    table = w.table()
+    oracle.build()
+    t0 = time.perf_counter()
+    _, pairs = oracle.convolve(x, table, w.theta_cut, level=1, pixels=pix, return_pairs=True)
+    dt = time.perf_counter() - t0
+    return pairs, dt, oracle.max_threads()
+
+
+def run_reference(args, w: wl.Workload):
+    """--impl reference: the oracle on the host cores, bounded sample per step (tier contract ④)."""
+    rank, _, world = replicas.env_world()
+    if rank != 0:
+        return
+    n_pix = args.ref_pixels
+    for _ in range(args.warmup):
+        oracle_sample(w, max(1024, n_pix // 16), 777)
+    pairs_total, t_total, cores = 0, 0.0, 1
+    for s in range(args.steps):
+        pairs, dt, cores = oracle_sample(w, n_pix, 1000 + s)
+        pairs_total += pairs; t_total += dt
+    value = pairs_total / t_total
+    sample = f"{n_pix} seeded uniform random output pixels of {w.name} per step, oracle level 1 (windowed brute force)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w),
+        "output_pixels_per_s": n_pix * args.steps / t_total,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w: wl.Workload):
+    return {"workload": w.name, "n_theta": w.n_theta, "n_phi": w.n_phi,
+            "theta_cut_arcmin": w.theta_cut / wl.ARCMIN, "kernel": w.kernel,
+            "fwhm_arcmin": w.sigma / wl.FWHM_TO_SIGMA / wl.ARCMIN, "n_table": w.n_table,
+            "maps_per_step": 1, "parallelism": "replicas (no sharding, SURVEY 8(e))",
+            "l2": "map in+out = %.0f MB per step vs 126 MB L2: %s" % (
+                8e-6 * w.n_pix, "larger than L2, no flush needed" if 8 * w.n_pix > 126e6 else "input buffers rotated")}
+
+
+def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True):
+    import torch
+    from paper_1211_3556_b200 import arkcos
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    hbm_gbs, sm_max_mhz, peak_src = load_peaks()
+    table = w.table()
+    x32 = w.map_f32()
+    plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut)
+    info = plan.info()
+    stream = torch.cuda.Stream(device=dev)
+    sh = stream.cuda_stream
+    # rotate input buffers when the map would otherwise sit in L2 between steps
+    n_rot = 1 if 8 * w.n_pix > 126e6 else max(2, int(math.ceil(260e6 / (4 * w.n_pix))))
+    d_in = [torch.from_numpy(x32).to(dev) for _ in range(n_rot)]
+    d_out = torch.empty_like(d_in[0])
+    with torch.cuda.stream(stream):
+        for i in range(warmup):
+            plan.convolve(d_in[i % n_rot], d_out, sh)
+    stream.synchronize()
+
+    # ---- timed region: K back-to-back steps, CUDA events on the launching stream --------------------
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    replicas.barrier(dist)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for i in range(steps):
+            plan.convolve(d_in[i % n_rot], d_out, sh)
+        e1.record(stream)
+    stream.synchronize()
+    torch.cuda.synchronize()
+    replicas.barrier(dist)
+    elapsed_ms = e0.elapsed_time(e1)
+    # ---- per-kernel device times (CUDA events inside the library, same stream), K more steps --------
+    gen_ms, conv_ms = [], []
+    for i in range(steps):
+        g, c = plan.convolve_timed(d_in[i % n_rot], d_out, sh)
+        gen_ms.append(g); conv_ms.append(c)
+    clocks = sampler.stop()
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if want_e2e:
+        h_in = torch.from_numpy(x32).pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        hi, ho = h_in.numpy(), h_out.numpy()
+        for _ in range(min(warmup, 2)):
+            plan.convolve_host(hi, ho, sh)
+        n_e2e = max(1, min(steps, 10))
+        replicas.barrier(dist)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            plan.convolve_host(hi, ho, sh)      # returns after the result is in host memory
+        e2e_ms = 1e3 * (time.perf_counter() - t0) / n_e2e
+        checksum = float(np.abs(ho[:: max(1, w.n_theta // 64)]).sum())
+        e2e = {"ms_per_step": e2e_ms, "steps": n_e2e, "checksum": checksum}
+
+    result = {"elapsed_ms": elapsed_ms, "gen_ms": float(np.mean(gen_ms)), "conv_ms": float(np.mean(conv_ms)),
+              "conv_ms_min": float(np.min(conv_ms)), "clocks": clocks, "info": info, "e2e": e2e,
+              "hbm_gbs": hbm_gbs, "sm_max_mhz": sm_max_mhz, "peak_src": peak_src,
+              "device_name": torch.cuda.get_device_name(dev), "sm_count": info.sm_count}
+    plan.destroy()
+    return result
+
+
+def build_line(w, args, res, world, total_ms, total_units, cpu):
+    info = res["info"]
+    pair_evals = int(info.pair_evals)
+    ms_per_step = total_ms / args.steps
+    value = replicas.throughput(total_units, total_ms)
+    peak_tflops = res["sm_count"] * FP32_LANES_PER_SM * 2 * res["sm_max_mhz"] * 1e6 / 1e12
+    achieved_tflops = 2.0 * pair_evals / (res["conv_ms"] * 1e-3) / 1e12
+    hbm_achieved = 8.0 * w.n_pix / (res["conv_ms"] * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(w),
+        "output_pixels_per_s": world * w.n_pix * args.steps / (total_ms * 1e-3),
+        "pair_evals_per_map": pair_evals,
+        "kernel_ms": {"generate_weights": res["gen_ms"], "convolve": res["conv_ms"], "convolve_min": res["conv_ms_min"]},
+        "roofline": {
+            "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+            "frac": achieved_tflops / peak_tflops, "traffic": ncu_traffic(w.name),
+            "kernel": "k_convolve", "flops_per_launch": 2.0 * pair_evals,
+            "peak_source": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json)" % (
+                res["sm_count"], res["sm_max_mhz"], res["peak_src"]),
+            "issued_lane_frac": float(info.fma_slots) / (res["conv_ms"] * 1e-3) / (peak_tflops * 1e12 / 2.0),
+            "hbm": {"achieved": hbm_achieved, "peak": res["hbm_gbs"], "unit": "GB/s", "frac": hbm_achieved / res["hbm_gbs"],
+                    "algorithmic_bytes_per_launch": 8.0 * w.n_pix},
+        },
+        "clocks": res["clocks"],
+        "gpu_launches": args.steps * int(info.kernels_per_convolve),
+        "device": res["device_name"],
+    }
+    if res["e2e"] is not None:
+        e = res["e2e"]
+        line["e2e"] = {"value": world * pair_evals / (e["ms_per_step"] * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": 4 * w.n_pix, "d2h_bytes_per_step": 4 * w.n_pix,
+                       "ms_per_step": e["ms_per_step"], "steps": e["steps"], "host_memory": "pinned",
+                       "api": "arkcos_convolve_host"}
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    return line
+
+
+def cpu_baseline(w: wl.Workload, n_pixels: int):
+    pairs, dt, cores = oracle_sample(w, n_pixels, 4242)
+    return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n_pixels} seeded uniform random output pixels of {w.name} ({pairs} pair evals in {dt:.1f} s), "
+                      "oracle level 1, OpenMP dynamic",
+            "output_pixels_per_s": n_pixels / dt}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--cpu-pixels", type=int, default=1 << 20, help="oracle sample size of the cpu_baseline leg")
+    ap.add_argument("--ref-pixels", type=int, default=1 << 17, help="oracle sample per step of --impl reference")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="five-config report + cost-vs-theta_cut curve")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = wl.by_name(args.workload)
+
+    if args.impl == "reference":
+        run_reference(args, w)
+        return 0
+
+    rank, local_rank, world = replicas.env_world()
+    dist = replicas.init("nccl")
+    import torch
+    dev = torch.device("cuda", local_rank)
+
+    if args.sweep:
+        if rank == 0:
+            sweep(args)
+        return 0
+
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False)
+    units = float(res["info"].pair_evals) * args.steps
+    total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
+    if rank == 0:
+        cpu = None if (args.no_cpu or world > 1) else cpu_baseline(w, args.cpu_pixels)
+        print(json.dumps(build_line(w, args, res, world, total_ms, total_units, cpu)), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def sweep(args):
+    """All five configs: throughput, roofline fractions, and GPU time vs theta_cut with both fits
+    (a*cut^2 + c, and the paper's linear form of Eq. 2.3)."""
+    curve = {}
+    for w in wl.all_workloads():
+        res = measure(w, max(3, args.steps // 2), 3, None, 0, want_cpu=False, want_e2e=False)
+        a = argparse.Namespace(**vars(args)); a.steps = max(3, args.steps // 2)
+        line = build_line(w, a, res, 1, res["elapsed_ms"], float(res["info"].pair_evals) * a.steps, None)
+        line["report"] = "sweep"
+        print(json.dumps(line), flush=True)
+        key = w.name.split("_cut")[0]
+        curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"]))
+    for key, pts in curve.items():
+        if len(pts) < 3:
+            continue
+        t = np.array([p[0] for p in pts]); ms = np.array([p[1] for p in pts])
+        quad = np.linalg.lstsq(np.stack([t ** 2, np.ones_like(t)], 1), ms, rcond=None)[0]
+        lin = np.linalg.lstsq(np.stack([t, np.ones_like(t)], 1), ms, rcond=None)[0]
+        print(json.dumps({"report": "cost_curve", "family": key, "theta_cut_arcmin": t.tolist(), "gpu_ms_per_map": ms.tolist(),
+                          "fit_quadratic_ms": {"a_per_arcmin2": quad[0], "c": quad[1],
+                                               "rms_resid": float(np.sqrt(np.mean((quad[0] * t ** 2 + quad[1] - ms) ** 2)))},
+                          "fit_linear_ms": {"a_per_arcmin": lin[0], "c": lin[1],
+                                            "rms_resid": float(np.sqrt(np.mean((lin[0] * t + lin[1] - ms) ** 2)))},
+                          "paper_eq_2_3": "t = 0.0232 s * theta_cut[arcmin] + 2.428 s (GTX 480, HEALPix nside 2048; context only)"}),
+              flush=True)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
