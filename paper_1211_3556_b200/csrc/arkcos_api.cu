@@ -39,7 +39,8 @@ struct arkcos_plan {
     PairDesc* d_pairs = nullptr;
     Item* d_items = nullptr;
     GenUnit* d_units = nullptr;
-    double *d_sin_t = nullptr, *d_area = nullptr, *d_a_r = nullptr, *d_s2 = nullptr, *d_table = nullptr;
+    double *d_s2 = nullptr, *d_table = nullptr;
+    uint32_t *d_ring_w_off = nullptr, *d_ring_slots = nullptr;
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging, lazily allocated
     size_t device_bytes = 0;
@@ -64,13 +65,11 @@ arkcos_status upload(arkcos_plan* pl, T** dst, const std::vector<T>& src) {
 
 arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
     GenParams g;
-    g.pairs = pl->d_pairs; g.units = pl->d_units; g.sin_t = pl->d_sin_t; g.area = pl->d_area;
-    g.a_r = pl->d_a_r; g.s2 = pl->d_s2; g.table = pl->d_table; g.weights = pl->d_weights;
-    g.n_units = (int)pl->sched.gen_units.size(); g.n_theta = pl->sched.n_theta; g.n_phi = pl->sched.n_phi;
-    g.n_table = pl->n_table; g.R = pl->sched.R;
+    g.units = pl->d_units; g.s2 = pl->d_s2; g.table = pl->d_table; g.weights = pl->d_weights;
+    g.n_units = (int)pl->sched.gen_units.size(); g.n_phi = pl->sched.n_phi; g.n_table = pl->n_table;
     g.t_scale = (double)(pl->n_table - 1) / pl->sched.theta_cut;
     g.table_in_smem = pl->table_in_smem;
-    k_generate_weights<<<pl->gen_grid, 256, pl->gen_smem, st>>>(g);
+    k_generate_weights<<<pl->gen_grid, kGenThreads, pl->gen_smem, st>>>(g);
     CU(cudaGetLastError());
     return ARKCOS_OK;
 }
@@ -78,7 +77,8 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
 arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
-    c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R;
+    c.ring_w_off = pl->d_ring_w_off; c.ring_slots = pl->d_ring_slots;
+    c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
     c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
     dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
     k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
@@ -122,8 +122,8 @@ const char* arkcos_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!pl) return ARKCOS_OK;
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
-        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_sin_t);
-        cudaFree(pl->d_area); cudaFree(pl->d_a_r); cudaFree(pl->d_s2); cudaFree(pl->d_table);
+        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_ring_w_off);
+        cudaFree(pl->d_ring_slots); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
         for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
         (void)cudaGetLastError();
@@ -165,9 +165,8 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
         if ((st = upload(pl, &pl->d_pairs, s.pairs)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_items, s.items)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_units, s.gen_units)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_sin_t, s.sin_t)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_area, s.area)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_a_r, s.a_r)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_ring_w_off, s.ring_w_off)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_ring_slots, s.ring_slots)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_s2, s.s2)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_table, pl->table)) != ARKCOS_OK) break;
         {
@@ -178,10 +177,7 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
             pl->device_bytes += bytes;
         }
         // launch configuration
-        int f_max = 0;
-        for (const Item& it : s.items) f_max = it.f_log2 > f_max ? it.f_log2 : f_max;
-        size_t smem = 0;
-        for (int fl = 0; fl <= f_max; fl++) { size_t b = conv_smem_bytes(fl); smem = b > smem ? b : smem; }
+        const size_t smem = s.smem_bytes;
         pl->conv_smem = smem;
         if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                      "cudaFuncSetAttribute(k_convolve)")) { st = ARKCOS_ECUDA; break; }
@@ -191,8 +187,9 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
         if (!cuda_ok(cudaFuncSetAttribute(k_generate_weights, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)(pl->gen_smem > 0 ? pl->gen_smem : 1)),
                      "cudaFuncSetAttribute(k_generate_weights)")) { st = ARKCOS_ECUDA; break; }
-        int units = (int)s.gen_units.size();
-        pl->gen_grid = units < pl->sm_count ? (units > 0 ? units : 1) : pl->sm_count;
+        const int units = (int)s.gen_units.size(), per_cta = kGenThreads / 32;
+        const int want = (units + per_cta - 1) / per_cta;
+        pl->gen_grid = want < pl->sm_count ? (want > 0 ? want : 1) : pl->sm_count;
         for (auto& e : pl->ev)
             if (!cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) { st = ARKCOS_ECUDA; break; }
         if (st != ARKCOS_OK) break;

@@ -17,11 +17,15 @@ constexpr int kP = 16;                 // outputs per thread in phi (register-bl
 constexpr int kWarpSpan = 32 * kP;     // 512 contiguous phi outputs per warp
 constexpr int kWarps = 8;              // warps per CTA
 constexpr int kThreads = 32 * kWarps;
-constexpr int kMaxF = 8;               // a CTA covers F phi sub-tiles x S = kWarps/F tap splits
-constexpr int kGenUnitTaps = 1024;     // taps per weight-generator work unit
+constexpr int kHaloNarrow = 32;        // narrow rings: every stored tap window lies inside [-32, 32)
+constexpr int kPrefetchWide = 3;       // float4 pairs a thread holds in registers for the next wide stage
+constexpr int kPrefetchNarrow = 5;     // ... for the next narrow pass (S new rows)
+constexpr int kGenUnitTaps = 1024;     // taps per weight-generator work unit (one warp)
+constexpr int kSmemBudget = 220 * 1024;
 
-// Tap block (taps staged per shared-memory fill) as a function of log2(F).
-ARKCOS_HD constexpr int tap_block(int f_log2) { return f_log2 == 3 ? 512 : (f_log2 == 2 ? 1024 : 2048); }
+// Tap block (taps staged per shared-memory fill of a WIDE item) as a function of log2(F), chosen so
+// that one stage (2 + L + TB + 2 pairs at most) is at most kPrefetchWide * kThreads = 768 quads.
+ARKCOS_HD constexpr int tap_block(int f_log2) { return f_log2 >= 2 ? 1016 : (f_log2 == 1 ? 2040 : 2048); }
 
 // One (north output ring i, input ring j = i + r) pair.  The southern mirror pair
 // (n_theta-1-i, n_theta-1-j) has identical weights and is computed by the same CTA (FFMA2 lanes).
@@ -32,17 +36,26 @@ struct PairDesc {
     int32_t half;     // D (taps -D..D inside theta_cut); n_phi = whole ring; -1 = empty
 };
 
+enum ItemKind : int16_t { kWide = 0, kNarrow = 1 };
+
 // One CTA of the convolution launch.
 struct Item {
-    int32_t i_north;  // output ring in the northern half; the CTA also produces ring n_theta-1-i
+    int32_t i0;       // first northern output ring (the CTA also produces the mirror rings)
     int32_t k0;       // first output phi of the tile
-    int32_t f_log2;   // F = 1 << f_log2 sub-tiles of 512 outputs; S = kWarps / F tap splits
-    int32_t row_lo;   // first input-row slot r (0..2R) this CTA sums (cluster splitting; 0 in v1)
+    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles of 512 outputs; S = kWarps / F
+    int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings, S rings per pass
+    int32_t nrings;
 };
 
+// Work unit of the weight generator (one warp): `count` taps d0, d0+1, ... of one ring pair.
 struct GenUnit {
-    uint32_t pair;    // index into the PairDesc array
-    uint32_t e0;      // first stored tap of the unit
+    uint32_t w_base;  // destination offset in the weight buffer
+    int32_t d0;       // first dphi index
+    int32_t count;    // taps to write (<= kGenUnitTaps)
+    int32_t half;     // D, or n_phi for a whole ring
+    double a;         // sin^2((t_i - t_j)/2)
+    double b;         // sin t_i sin t_j
+    double area;      // A_j
 };
 
 // Host-side result of step S1 (the ring-pair scheduler).  FP64 throughout.
@@ -57,8 +70,14 @@ struct Schedule {
     std::vector<double> a_r;                // [R+1] sin^2(r dtheta / 2)
     std::vector<double> s2;                 // [n_phi/2+1] sin^2(d dphi / 2)
     std::vector<PairDesc> pairs;            // [n_north][2R+1]
+    std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
+    std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows)
     std::vector<Item> items;                // cost-sorted, heaviest first
     std::vector<GenUnit> gen_units;
+    int first_narrow = 0;                   // rings [first_narrow, n_north) use the narrow kernel path
+    int narrow_f_log2 = 0;                  // F of the narrow items
+    int narrow_wslot = 0;                   // floats per ring in the narrow weight buffers
+    size_t smem_bytes = 0;                  // dynamic shared memory of the convolution launch
     unsigned long long pair_evals = 0;      // useful FMAs per map
     unsigned long long weights = 0;         // in-support weights, no symmetry reduction
     unsigned long long fma_slots = 0;       // FMA lanes issued per map (padding included)
@@ -72,6 +91,10 @@ struct Schedule {
         return &pairs[(size_t)i_north * (2 * R + 1) + r];
     }
 };
+
+// shared memory of one WIDE item with tile factor f_log2 (two stage buffers), and of the NARROW path
+size_t wide_smem_bytes(int f_log2, int R);
+size_t narrow_smem_bytes(int f_log2, int R, int wslot);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
 int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);

@@ -101,39 +101,112 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     }
     s.weight_slots = w_off;
 
-    // ---- generator work units -------------------------------------------------------------------
-    for (size_t pi = 0; pi < s.pairs.size(); pi++)
-        for (int e0 = 0; e0 < s.pairs[pi].ntaps; e0 += kGenUnitTaps) s.gen_units.push_back(GenUnit{(uint32_t)pi, (uint32_t)e0});
+    // ring-contiguous weight blocks (rows r = -R..R of one ring are stored back to back)
+    s.ring_w_off.assign(s.n_north, 0u); s.ring_slots.assign(s.n_north, 0u);
+    for (int i = 0; i < s.n_north; i++) {
+        bool first = true;
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (p.ntaps == 0) continue;
+            if (first) { s.ring_w_off[i] = p.w_off; first = false; }
+        }
+        s.ring_slots[i] = (uint32_t)ring_slots[i];
+    }
 
-    // ---- work items: (north ring, phi tile), tile width 512 F chosen so that no item exceeds
-    //      ~1/6 of one SM's share of the whole job; heaviest first (H1: polar imbalance) ------------
-    unsigned long long total = 0;
-    for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi;
-    double c_max = (double)total / (double)sm_count / 6.0;
-    struct Tmp { Item it; double cost; };
-    std::vector<Tmp> tmp;
+    // ---- generator work units: one warp writes up to kGenUnitTaps taps of one ring pair -----------
+    for (int i = 0; i < s.n_north; i++)
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            const int j = i + r - s.R;
+            for (int e0 = 0; e0 < p.ntaps; e0 += kGenUnitTaps) {
+                GenUnit g;
+                g.w_base = p.w_off + (uint32_t)e0; g.d0 = p.start + e0;
+                g.count = std::min(kGenUnitTaps, p.ntaps - e0); g.half = p.half;
+                g.a = s.a_r[std::abs(r - s.R)]; g.b = s.sin_t[i] * s.sin_t[j]; g.area = s.area[j];
+                s.gen_units.push_back(g);
+            }
+        }
+
+    // ---- ring classes -----------------------------------------------------------------------------
+    // NARROW rings: every stored window lies inside [-kHaloNarrow, kHaloNarrow).  Windows widen
+    // towards the pole, so the narrow rings are the band [first_narrow, n_north) next to the equator.
     int f_cap = 0;                                            // largest useful F for this n_phi
     while (f_cap < 3 && (kWarpSpan << f_cap) < n_phi) f_cap++;
-    for (int i = 0; i < s.n_north; i++) {
-        if (ring_slots[i] == 0) {
-            // ring with no work still needs its output zeroed: one cheap item per tile
+    auto ring_is_narrow = [&](int i) {
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (p.ntaps == 0) continue;
+            if (p.half == n_phi || p.start < -kHaloNarrow || p.start + p.ntaps > kHaloNarrow) return false;
         }
-        int fl = f_cap;
+        return true;
+    };
+    s.first_narrow = s.n_north;
+    while (s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
+    unsigned long long wslot = 0;
+    for (int i = s.first_narrow; i < s.n_north; i++) wslot = std::max<unsigned long long>(wslot, ring_slots[i]);
+    s.narrow_wslot = (int)((wslot + 3) & ~3ull);
+    s.narrow_f_log2 = -1;
+    for (int fl = f_cap; fl >= 0; fl--)
+        if (narrow_smem_bytes(fl, s.R, s.narrow_wslot) <= (size_t)kSmemBudget) { s.narrow_f_log2 = fl; break; }
+    if (s.narrow_f_log2 < 0 || s.n_north - s.first_narrow < 1) { s.first_narrow = s.n_north; s.narrow_f_log2 = 0; }
+
+    // ---- work items, heaviest first (H1: polar imbalance) -------------------------------------------
+    unsigned long long total = 0;
+    for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi;
+    const double c_max = (double)total / (double)sm_count / 8.0;   // no item above 1/8 of an SM's share, if possible
+    struct Tmp { Item it; double cost; };
+    std::vector<Tmp> tmp;
+    size_t smem = 0;
+    // WIDE: (ring, phi tile of 512 F), F <= 4
+    for (int i = 0; i < s.first_narrow; i++) {
+        int fl = std::min(f_cap, 2);
         while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWarpSpan << fl) > c_max) fl--;
-        int L = kWarpSpan << fl;
+        const int L = kWarpSpan << fl;
+        smem = std::max(smem, wide_smem_bytes(fl, s.R));
         for (int k0 = 0; k0 < n_phi; k0 += L) {
-            int span = std::min(L, n_phi - k0);
-            double cost = (double)ring_slots[i] * (double)L + 2000.0;   // issued slots, not useful ones
-            tmp.push_back(Tmp{Item{i, k0, fl, 0}, cost});
-            // both mirror rings: 2 FMA lanes per slot (one FFMA2)
-            s.fma_slots += 2ull * ring_slots[i] * (unsigned long long)L;
-            (void)span;
+            tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kWide, 1}, (double)ring_slots[i] * (double)L + 4000.0});
+            s.fma_slots += 2ull * ring_slots[i] * (unsigned long long)L;      // x2: both mirror rings
         }
     }
+    // NARROW: (band of B rings, phi tile of 512 F); S = 8/F rings advance together
+    if (s.first_narrow < s.n_north) {
+        const int fl = s.narrow_f_log2, S = kWarps >> fl, L = kWarpSpan << fl;
+        smem = std::max(smem, narrow_smem_bytes(fl, s.R, s.narrow_wslot));
+        const int b_min = ((2 * (2 * s.R + S)) + S - 1) / S * S;       // keep the band prologue below ~50 % extra staging
+        int i = s.first_narrow;
+        while (i < s.n_north) {
+            double c = 0.0; int b = 0;
+            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += (double)ring_slots[i + b] * (double)L; b++; }
+            b = std::min((b + S - 1) / S * S, s.n_north - i);
+            if (s.n_north - (i + b) < b_min / 2) b = s.n_north - i;     // do not leave a tiny tail band
+            c = 0.0;
+            for (int q = 0; q < b; q++) c += (double)ring_slots[i + q] * (double)L;
+            for (int k0 = 0; k0 < n_phi; k0 += L) {
+                tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, b}, c + 4000.0});
+                for (int q = 0; q < b; q++) s.fma_slots += 2ull * ring_slots[i + q] * (unsigned long long)L;
+            }
+            i += b;
+        }
+    }
+    s.smem_bytes = smem;
     std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
     s.items.reserve(tmp.size());
     for (auto& t : tmp) s.items.push_back(t.it);
     return 0;
+}
+
+size_t wide_smem_bytes(int f_log2, int R) {
+    const int L = kWarpSpan << f_log2, TB = tap_block(f_log2);
+    const size_t cap_pairs = (size_t)((L + TB + 8 + 15) & ~15);
+    const size_t stage = 2 * (cap_pairs * 8 + (size_t)TB * 4) + (size_t)(2 * R + 1) * sizeof(PairDesc);
+    const size_t red = (size_t)kWarps * kP * 32 * 8;
+    return stage > red ? stage : red;
+}
+
+size_t narrow_smem_bytes(int f_log2, int R, int wslot) {
+    const int S = kWarps >> f_log2;
+    const size_t slot_pairs = (size_t)(kWarpSpan << f_log2) + 2 * kHaloNarrow;
+    return (size_t)(2 * R + S) * slot_pairs * 8 + 2ull * S * (size_t)wslot * 4 + 2ull * S * (2 * R + 1) * sizeof(PairDesc);
 }
 
 }  // namespace arkcos
