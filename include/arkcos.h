@@ -53,6 +53,11 @@ typedef enum {
  * streams concurrently; on-the-fly plans rewrite the (identical) weights in each call and must not
  * be used from two streams at the same time. */
 #define ARKCOS_PLAN_CACHE_WEIGHTS 2u
+/* Measurement hooks: launch only the WIDE (polar / high-latitude rings) or only the NARROW
+ * (equatorial band) work items of step S3, to time the two kernel paths separately.  The output
+ * rings of the other class are NOT written.  Never set both. */
+#define ARKCOS_PLAN_ONLY_WIDE 4u
+#define ARKCOS_PLAN_ONLY_NARROW 8u
 
 /*
  * arkcos_plan_create - step S1 (ring-pair scheduler, host FP64) and device uploads.
@@ -130,6 +135,9 @@ typedef struct {
     int sm_count;                        /* 0 for host-only plans                                 */
     unsigned flags;
     unsigned long long device_bytes;     /* device memory owned by the plan                       */
+    unsigned long long fma_slots_wide;   /* part of fma_slots issued by the WIDE work items       */
+    int first_narrow_ring;               /* northern rings [first_narrow_ring, ceil(n_theta/2))   */
+                                         /*   and their mirrors take the NARROW path              */
 } arkcos_plan_info;
 arkcos_status arkcos_plan_get_info(const arkcos_plan *plan, arkcos_plan_info *info);
 

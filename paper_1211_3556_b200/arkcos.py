@@ -17,6 +17,7 @@ from . import build as _build
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 PLAN_DEFAULT, PLAN_HOST_ONLY, PLAN_CACHE_WEIGHTS = 0, 1, 2
+PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos.h)
 
 _c_plan_p = ctypes.c_void_p
 
@@ -28,7 +29,8 @@ class PlanInfo(ctypes.Structure):
                 ("fma_slots", ctypes.c_ulonglong), ("weight_slots", ctypes.c_ulonglong),
                 ("n_items", ctypes.c_int), ("n_gen_units", ctypes.c_int),
                 ("kernels_per_convolve", ctypes.c_int), ("sm_count", ctypes.c_int),
-                ("flags", ctypes.c_uint), ("device_bytes", ctypes.c_ulonglong)]
+                ("flags", ctypes.c_uint), ("device_bytes", ctypes.c_ulonglong),
+                ("fma_slots_wide", ctypes.c_ulonglong), ("first_narrow_ring", ctypes.c_int)]
 
 
 class ArkcosError(RuntimeError):

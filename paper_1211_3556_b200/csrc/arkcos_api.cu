@@ -80,6 +80,7 @@ arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d
     c.ring_w_off = pl->d_ring_w_off; c.ring_slots = pl->d_ring_slots;
     c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
     c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
+    if (pl->sched.items.empty()) return ARKCOS_OK;
     dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
     k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
     CU(cudaGetLastError());
@@ -138,7 +139,8 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
     *plan = nullptr;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
-    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
+    if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
     arkcos_plan* pl = new (std::nothrow) arkcos_plan();
     if (!pl) return ARKCOS_ENOMEM;
@@ -157,6 +159,13 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
         }
         int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
         if (rc != 0) { delete pl; return (arkcos_status)rc; }
+        if (pl->sched.smem_bytes > (size_t)kSmemBudget) { delete pl; return ARKCOS_EUNSUPPORTED; }
+        if (flags & (ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) {     // measurement hooks
+            const int keep = (flags & ARKCOS_PLAN_ONLY_WIDE) ? kWide : kNarrow;
+            std::vector<Item> kept;
+            for (const Item& it : pl->sched.items) if (it.kind == keep) kept.push_back(it);
+            pl->sched.items.swap(kept);
+        }
     } catch (const std::bad_alloc&) { delete pl; return ARKCOS_ENOMEM; }
     if (flags & ARKCOS_PLAN_HOST_ONLY) { *plan = pl; return ARKCOS_OK; }
 
@@ -281,6 +290,7 @@ arkcos_status arkcos_plan_get_info(const arkcos_plan* pl, arkcos_plan_info* info
     info->n_items = (int)s.items.size(); info->n_gen_units = (int)s.gen_units.size();
     info->kernels_per_convolve = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) ? 1 : 2;
     info->sm_count = pl->sm_count; info->flags = pl->flags; info->device_bytes = pl->device_bytes;
+    info->fma_slots_wide = s.fma_slots_wide; info->first_narrow_ring = s.first_narrow;
     return ARKCOS_OK;
 }
 
@@ -309,13 +319,15 @@ arkcos_status arkcos_plan_pair_weights(const arkcos_plan* pl, int i, int j, floa
     CU(cudaDeviceSynchronize());
     int dmax = pd->half == s.n_phi ? s.n_phi / 2 : pd->half;
     int cnt = dmax + 1 < cap ? dmax + 1 : cap;
-    std::vector<float> all(pd->ntaps);
-    CU(cudaMemcpy(all.data(), pl->d_weights + pd->w_off, sizeof(float) * pd->ntaps, cudaMemcpyDeviceToHost));
+    const bool eo = in_ < s.first_narrow;                     // wide ring: even/odd step layout (PairDesc)
+    const size_t floats = eo ? 2 * (size_t)pd->ntaps : (size_t)pd->ntaps;
+    std::vector<float> all(floats);
+    CU(cudaMemcpy(all.data(), pl->d_weights + pd->w_off, sizeof(float) * floats, cudaMemcpyDeviceToHost));
     for (int d = 0; d < cnt; d++) {
-        // tap +d is stored at e = d - start, except d = n_phi/2 of a whole ring, stored as d = -n_phi/2 (e = 0)
+        // tap +d is stored at e = d - start, except d = n_phi/2 of a whole ring, stored as d = -n_phi/2
         int e = d - pd->start;
-        if (e >= pd->ntaps) e = 0;
-        h_w[d] = all[e];
+        if (pd->half == s.n_phi && d == s.n_phi / 2) e = -d - pd->start;
+        h_w[d] = eo ? all[4 * (size_t)(e >> 1) + (e & 1)] : all[e];
     }
     *n = cnt;
     return ARKCOS_OK;

@@ -18,17 +18,27 @@ constexpr int kWarpSpan = 32 * kP;     // 512 contiguous phi outputs per warp
 constexpr int kWarps = 8;              // warps per CTA
 constexpr int kThreads = 32 * kWarps;
 constexpr int kHaloNarrow = 32;        // narrow rings: every stored tap window lies inside [-32, 32)
-constexpr int kPrefetchWide = 3;       // float4 pairs a thread holds in registers for the next wide stage
 constexpr int kPrefetchNarrow = 5;     // ... for the next narrow pass (S new rows)
 constexpr int kGenUnitTaps = 1024;     // taps per weight-generator work unit (one warp)
 constexpr int kSmemBudget = 220 * 1024;
 
-// Tap block (taps staged per shared-memory fill of a WIDE item) as a function of log2(F), chosen so
-// that one stage (2 + L + TB + 2 pairs at most) is at most kPrefetchWide * kThreads = 768 quads.
-ARKCOS_HD constexpr int tap_block(int f_log2) { return f_log2 >= 2 ? 1016 : (f_log2 == 1 ? 2040 : 2048); }
+// ---- WIDE items (windows of 64 .. n_phi taps): warp-autonomous even/odd-tap path -----------------
+// A warp owns kWideSpan contiguous outputs of ONE ring (32 per lane) and streams its share of the
+// ring's taps through a private, double-buffered shared-memory stage of kWideStage tap pairs.
+constexpr int kWideP = 32;                          // outputs per lane
+constexpr int kWideSpan = 32 * kWideP;              // 1024 outputs per warp
+constexpr int kWideStage = 128;                     // tap pairs ("steps") per stage; even
+constexpr int kWideZChunks = 368;                   // 16-byte chunks of a stage's input window: (1024 + 2*128 + 4)/4 = 321
+                                                    //   logical chunks, one pad chunk after every 8 (lane stride 9 chunks)
+constexpr int kWideWBytes = (kWideStage + 4) * 16;  // weights of a stage: 16 bytes per step (+ prefetch slack)
+constexpr int kWideStageBytes = kWideZChunks * 16 + kWideWBytes;
 
 // One (north output ring i, input ring j = i + r) pair.  The southern mirror pair
-// (n_theta-1-i, n_theta-1-j) has identical weights and is computed by the same CTA (FFMA2 lanes).
+// (n_theta-1-i, n_theta-1-j) has identical weights.
+//   NARROW rings: `ntaps` FP32 weights w[e], tap e <-> dphi index d = start + e.
+//   WIDE rings:   ntaps/2 steps of 4 floats (K(d), K(d+1), K(d-1), K(d)), d = start + 2t: the weight
+//                 pairs of the even and of the odd outputs for the aligned input pair (x[d], x[d+1]);
+//                 2*ntaps floats in all; start is a multiple of 4.
 struct PairDesc {
     uint32_t w_off;   // offset, in floats, of the stored weights; multiple of 4
     int32_t start;    // dphi index d of stored tap 0 (even, <= 0)
@@ -40,22 +50,27 @@ enum ItemKind : int16_t { kWide = 0, kNarrow = 1 };
 
 // One CTA of the convolution launch.
 struct Item {
-    int32_t i0;       // first northern output ring (the CTA also produces the mirror rings)
+    int32_t i0;       // kWide: the output ring (either hemisphere).  kNarrow: first NORTHERN output ring
+                      //   (the CTA also produces the mirror rings)
     int32_t k0;       // first output phi of the tile
-    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles of 512 outputs; S = kWarps / F
+    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles (kWideSpan outputs wide, 512 narrow); S = kWarps / F
     int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings, S rings per pass
     int32_t nrings;
 };
 
-// Work unit of the weight generator (one warp): `count` taps d0, d0+1, ... of one ring pair.
+// Work unit of the weight generator (one warp) for one ring pair.
+//   eo == 0: `count` taps d0, d0+1, ...            -> count floats
+//   eo == 1: `count` steps d = d0, d0+2, ...       -> 4 count floats (K(d), K(d+1), K(d-1), K(d))
 struct GenUnit {
     uint32_t w_base;  // destination offset in the weight buffer
     int32_t d0;       // first dphi index
-    int32_t count;    // taps to write (<= kGenUnitTaps)
+    int32_t count;    // taps / steps to write (<= kGenUnitTaps)
     int32_t half;     // D, or n_phi for a whole ring
     double a;         // sin^2((t_i - t_j)/2)
     double b;         // sin t_i sin t_j
     double area;      // A_j
+    int32_t eo;       // layout, see above
+    int32_t pad_;
 };
 
 // Host-side result of step S1 (the ring-pair scheduler).  FP64 throughout.
@@ -81,6 +96,7 @@ struct Schedule {
     unsigned long long pair_evals = 0;      // useful FMAs per map
     unsigned long long weights = 0;         // in-support weights, no symmetry reduction
     unsigned long long fma_slots = 0;       // FMA lanes issued per map (padding included)
+    unsigned long long fma_slots_wide = 0;  // ... of which by the WIDE items
     unsigned long long weight_slots = 0;    // floats in the weight buffer
 
     // window of ring pair (i, j) for ANY i (southern rings through the mirror): -1 / D / n_phi
@@ -92,8 +108,8 @@ struct Schedule {
     }
 };
 
-// shared memory of one WIDE item with tile factor f_log2 (two stage buffers), and of the NARROW path
-size_t wide_smem_bytes(int f_log2, int R);
+// shared memory of a WIDE item (two private stage buffers per warp), and of the NARROW path
+size_t wide_smem_bytes(int R);
 size_t narrow_smem_bytes(int f_log2, int R, int wslot);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).

@@ -14,9 +14,10 @@ namespace arkcos {
 //   w_ij[d] = A_j * K(gamma_ij(d)),  sin^2(gamma/2) = sin^2((t_i-t_j)/2) + sin t_i sin t_j sin^2(d dphi/2)
 //   (the cancellation-free form of cos(gamma) = cos t_i cos t_j + sin t_i sin t_j cos(d dphi), H3),
 //   K by LINEAR interpolation in the radial table held in shared memory, FP64 throughout, rounded
-//   once to FP32.  Output layout: for each northern ring pair, `ntaps` floats for taps
-//   d = start .. start+ntaps-1, zero outside |d| <= D (so the convolution kernel needs no masks).
-//   One warp per work unit; persistent CTAs so the table is loaded into shared memory once per SM.
+//   once to FP32; zero outside the window (so the convolution kernels need no masks).
+//   Output layouts (PairDesc): plain taps for the narrow rings, (K(d), K(d+1), K(d-1), K(d)) steps
+//   for the wide rings.  One warp per work unit; persistent CTAs so the table is loaded into shared
+//   memory once per SM.
 // ================================================================================================
 struct GenParams {
     const GenUnit* units;
@@ -30,6 +31,21 @@ struct GenParams {
 
 constexpr int kGenThreads = 512;
 
+__device__ __forceinline__ float gen_weight(const GenParams& p, const GenUnit& g, const double* tab, const int d) {
+    const int ad = d < 0 ? -d : d;
+    const bool inside = (g.half == p.n_phi) ? (d >= -(p.n_phi / 2) && d < p.n_phi / 2) : (ad <= g.half);
+    if (!inside) return 0.0f;
+    double h = fma(g.b, p.s2[ad], g.a);
+    h = fmin(h, 1.0);
+    const double gam = 2.0 * asin(sqrt(h));
+    const double t = gam * p.t_scale;
+    int m = (int)t;
+    m = min(m, p.n_table - 2);
+    const double f = t - (double)m;
+    const double k = (1.0 - f) * tab[m] + f * tab[m + 1];
+    return (float)(g.area * k);
+}
+
 __global__ void __launch_bounds__(kGenThreads) k_generate_weights(const GenParams p) {
     extern __shared__ double s_table[];
     const double* tab = p.table;
@@ -41,23 +57,21 @@ __global__ void __launch_bounds__(kGenThreads) k_generate_weights(const GenParam
     const int warps = kGenThreads / 32, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int u = blockIdx.x * warps + warp; u < p.n_units; u += gridDim.x * warps) {
         const GenUnit g = p.units[u];
-        const bool whole = (g.half == p.n_phi);
-        for (int e = lane; e < g.count; e += 32) {
-            const int d = g.d0 + e;
-            const int ad = d < 0 ? -d : d;
-            float w = 0.0f;
-            if (whole || ad <= g.half) {
-                double h = fma(g.b, p.s2[ad], g.a);
-                h = fmin(h, 1.0);
-                const double gam = 2.0 * asin(sqrt(h));
-                const double t = gam * p.t_scale;
-                int m = (int)t;
-                m = min(m, p.n_table - 2);
-                const double f = t - (double)m;
-                const double k = (1.0 - f) * tab[m] + f * tab[m + 1];
-                w = (float)(g.area * k);
+        if (g.eo == 0) {
+            for (int e = lane; e < g.count; e += 32) p.weights[(size_t)g.w_base + e] = gen_weight(p, g, tab, g.d0 + e);
+        } else {
+            // step t: d = d0 + 2t.  K(d-1) of a lane is K(d+1) of the lane before it.
+            float carry = gen_weight(p, g, tab, g.d0 - 1);
+            for (int e0 = 0; e0 < g.count; e0 += 32) {
+                const int e = e0 + lane;
+                const int d = g.d0 + 2 * e;
+                float k0 = 0.f, k1 = 0.f;
+                if (e < g.count) { k0 = gen_weight(p, g, tab, d); k1 = gen_weight(p, g, tab, d + 1); }
+                float km = __shfl_up_sync(0xffffffffu, k1, 1);
+                if (lane == 0) km = carry;
+                carry = __shfl_sync(0xffffffffu, k1, 31);
+                if (e < g.count) *reinterpret_cast<float4*>(p.weights + (size_t)g.w_base + 4 * (size_t)e) = make_float4(k0, k1, km, k0);
             }
-            p.weights[(size_t)g.w_base + e] = w;
         }
     }
 }
@@ -193,135 +207,191 @@ __device__ __forceinline__ void store_outputs(const ConvParams& p, float* out, i
 }
 
 // ------------------------------------------------------------------------------------------------
-// WIDE item
+// WIDE item: one output ring (either hemisphere), F sub-tiles of kWideSpan outputs x S tap splits.
+//
+// Every warp is autonomous: it streams ITS share of the ring's taps through two private stage buffers
+// filled with cp.async (no CTA barrier until the final reduction of the S splits), so the warps of an
+// SM drift apart and the FMA pipe never waits for a common stage hand-over.
+//
+// Even/odd packing: a lane owns 32 consecutive outputs k..k+31.  For the aligned input pair
+// Z = (x[k+2m+d], x[k+2m+d+1]), d even, one FFMA2 with the weight pair (K(d), K(d+1)) advances the
+// EVEN output k+2m by two taps, and one with (K(d-1), K(d)) advances the ODD output k+2m+1; the two
+// halves of an accumulator are added at the end.  No input interleaving, no weight duplication:
+// the input rows are staged as they are in memory.
+//
+// Stage layout: logical float m of the stage = x[(phi0 + m) mod n_phi]; 16-byte chunk c sits at
+// physical chunk c + (c >> 3), i.e. lane tiles (8 chunks) have a stride of 9 chunks and LDS.128 is
+// conflict free without swizzle arithmetic.
 // ------------------------------------------------------------------------------------------------
-struct WideStage {       // one (row, tap block) of the item
-    int r, e0, nt;       // row slot 0..2R, first tap, taps in the block; r > 2R = end
-    int j;               // input ring
-    int phi4;            // float4-aligned phi of segment pair 0, in [0, n_phi)
-    int delta;           // 0 or 2: pair index of tap e0 for output k0
-    int nq;              // quads to stage
-    uint32_t w_off;      // weights of this block
-};
-
-__device__ __forceinline__ void wide_describe(const ConvParams& p, const Item& it, int L, WideStage& s, const PairDesc& pd) {
-    s.nt = min(tap_block(it.f_log2), pd.ntaps - s.e0);
-    s.j = it.i0 + s.r - p.R;
-    const int org = it.k0 + pd.start + s.e0;
-    const int org4 = org & ~3;
-    s.delta = org - org4;
-    s.phi4 = wrap_phi(org4, p.n_phi);
-    s.nq = (s.delta + L + s.nt - 1 + 3) >> 2;
-    s.w_off = pd.w_off + (uint32_t)s.e0;
+__device__ __forceinline__ void ffma2p(uint64_t& acc, const uint64_t z, const uint64_t w) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(z), "l"(w));
 }
-// first stage at or after (r, e0); the ring's pair descriptors are in shared memory
-__device__ __forceinline__ void wide_seek(const ConvParams& p, const Item& it, int L, WideStage& s, const PairDesc* spd) {
-    const int W = 2 * p.R + 1;
-    while (s.r < W) {
-        const PairDesc pd = spd[s.r];
-        if (s.e0 < pd.ntaps) { wide_describe(p, it, L, s, pd); return; }
-        s.r++; s.e0 = 0;
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int kZRing = 10;                // register window: 10 chunks = 20 input pairs (17 live + prefetch)
+
+// One double step (4 taps) at window phase PH.  Live chunks q .. q+8 sit in ring slots (PH + c) % 10;
+// chunk q+9 is fetched into the slot chunk q-1 has just left, weights of double step q+1 into wn.
+template <int PH>
+__device__ __forceinline__ void eo_dstep(uint64_t (&E)[16], uint64_t (&O)[16], uint64_t (&z)[2 * kZRing],
+                                         ulonglong2 (&w)[2], const char* __restrict__ zlane,
+                                         const ulonglong2* __restrict__ ws, const int q) {
+    const int u = q + 9;
+    const ulonglong2 nz = *reinterpret_cast<const ulonglong2*>(zlane + ((u + (u >> 3)) << 4));
+    const ulonglong2 wn0 = ws[2 * q + 2], wn1 = ws[2 * q + 3];
+#pragma unroll
+    for (int m = 0; m < 16; m++) {
+        ffma2p(E[m], z[(2 * PH + m) % (2 * kZRing)], w[0].x);
+        ffma2p(O[m], z[(2 * PH + m) % (2 * kZRing)], w[0].y);
+    }
+#pragma unroll
+    for (int m = 0; m < 16; m++) {
+        ffma2p(E[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[1].x);
+        ffma2p(O[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[1].y);
+    }
+    z[(2 * (PH + 9)) % (2 * kZRing)] = nz.x;
+    z[(2 * (PH + 9) + 1) % (2 * kZRing)] = nz.y;
+    w[0] = wn0; w[1] = wn1;
+}
+
+// E[m] += sum_t Z[m+t] * ws[t].x,  O[m] += sum_t Z[m+t] * ws[t].y  over t = 0 .. 2 nq - 1
+__device__ __forceinline__ void eo_taps(uint64_t (&E)[16], uint64_t (&O)[16], const char* __restrict__ zlane,
+                                        const ulonglong2* __restrict__ ws, const int nq) {
+    uint64_t z[2 * kZRing];
+#pragma unroll
+    for (int c = 0; c < 9; c++) {
+        const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(zlane + ((c + (c >> 3)) << 4));
+        z[2 * c] = v.x; z[2 * c + 1] = v.y;
+    }
+    z[18] = 0ull; z[19] = 0ull;
+    ulonglong2 w[2] = {ws[0], ws[1]};
+    int q = 0;
+    for (;;) {
+        eo_dstep<0>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<1>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<2>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<3>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<4>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<5>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<6>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<7>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<8>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
+        eo_dstep<9>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
     }
 }
+
+struct WideStage {
+    const float* row;    // input ring
+    int phi0;            // phi of logical float 0 of the stage, in [0, n_phi), multiple of 4
+    int nq;              // double steps (4 taps each), 1 .. kWideStage/2
+    uint32_t w_off;      // first weight of the stage (floats)
+};
 
 __device__ void conv_wide(const ConvParams& p, const Item& it, uint4* smem, const float* in, float* out) {
     const int F = 1 << it.f_log2, S = kWarps >> it.f_log2;
-    const int L = kWarpSpan << it.f_log2, TB = tap_block(it.f_log2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int f = warp & (F - 1), s = warp >> it.f_log2;
     const int W = 2 * p.R + 1;
-    const int cap_pairs = (L + TB + 8 + 15) & ~15;
-    const int buf_chunks = cap_pairs / 2 + TB / 4;           // one stage buffer: Z chunks then weights
-    const uint32_t lane_pair0 = (uint32_t)(f * kWarpSpan + lane * kP);
-    const int s_log2 = 3 - it.f_log2;
-    PairDesc* spd = reinterpret_cast<PairDesc*>(smem + 2 * buf_chunks);   // [W] descriptors of this ring
-    for (int r = threadIdx.x; r < W; r += kThreads) spd[r] = p.pairs[(size_t)it.i0 * W + r];
+    const int i = it.i0;
+    const bool mirrored = 2 * i >= p.n_theta;                  // southern ring: weights of its mirror pair
+    const int i_n = mirrored ? p.n_theta - 1 - i : i;
+    char* wsm = reinterpret_cast<char*>(smem) + (size_t)warp * 2 * kWideStageBytes;
+    PairDesc* spd = reinterpret_cast<PairDesc*>(reinterpret_cast<char*>(smem) + (size_t)kWarps * 2 * kWideStageBytes);
+    for (int r = threadIdx.x; r < W; r += kThreads) spd[r] = p.pairs[(size_t)i_n * W + r];
     __syncthreads();
 
-    uint64_t acc[kP];
-#pragma unroll
-    for (int q = 0; q < kP; q++) acc[q] = 0ull;
-
-    WideStage cur; cur.r = 0; cur.e0 = 0;
-    wide_seek(p, it, L, cur, spd);
-    int buf = 0;
-    // prologue: stage the first block directly
-    if (cur.r < W) {
-        uint4* zs = smem;
-        const float* row_n = in + (size_t)cur.j * p.n_phi;
-        const float* row_s = in + (size_t)(p.n_theta - 1 - cur.j) * p.n_phi;
-        for (int q = threadIdx.x; q < cur.nq; q += kThreads)
-            quad_store(zs, q, quad_load(row_n, row_s, wrap_phi(cur.phi4 + 4 * q, p.n_phi)));
-        float* ws = reinterpret_cast<float*>(smem + cap_pairs / 2);
-        for (int q = threadIdx.x; q < (cur.nt >> 2); q += kThreads) cp_async16(ws + 4 * q, p.weights + (size_t)cur.w_off + 4 * q);
-        cp_async_wait_all();
+    const int K0 = it.k0 + f * kWideSpan;                      // first output of this warp
+    // this warp's share [g_lo, g_hi) of the ring's double steps (rows concatenated)
+    int G = 0;
+    for (int r = 0; r < W; r++) G += spd[r].ntaps >> 2;
+    int g_lo = (int)(((long long)G * s) / S), g_hi = (int)(((long long)G * (s + 1)) / S);
+    if (K0 >= p.n_phi) g_hi = g_lo;                            // ragged tile: no outputs here
+    int r = 0, q = 0, remaining = g_hi - g_lo;
+    for (int acc = 0; r < W; r++) {
+        const int n = spd[r].ntaps >> 2;
+        if (g_lo < acc + n) { q = g_lo - acc; break; }
+        acc += n;
     }
-    __syncthreads();
-    while (cur.r < W) {
-        WideStage nxt; nxt.r = cur.r; nxt.e0 = cur.e0 + TB;
-        wide_seek(p, it, L, nxt, spd);
-        const bool more = nxt.r < W;
-        uint4* zs = smem + buf * buf_chunks;
-        const float* ws = reinterpret_cast<const float*>(zs + cap_pairs / 2);
-        uint4* zs_n = smem + (buf ^ 1) * buf_chunks;
-        float* ws_n = reinterpret_cast<float*>(zs_n + cap_pairs / 2);
-        // ---- prefetch the next stage: global loads into registers, weights by cp.async --------------
-        Quad pf[kPrefetchWide];
-        if (more) {
-            const float* row_n = in + (size_t)nxt.j * p.n_phi;
-            const float* row_s = in + (size_t)(p.n_theta - 1 - nxt.j) * p.n_phi;
+    auto next_stage = [&](WideStage& st) -> bool {
+        if (remaining <= 0) return false;
+        while (q >= (spd[r].ntaps >> 2)) { r++; q = 0; }
+        const PairDesc pd = spd[r];
+        st.nq = min(min(kWideStage / 2, (pd.ntaps >> 2) - q), remaining);
+        const int j = mirrored ? i - (r - p.R) : i + (r - p.R);
+        st.row = in + (size_t)j * p.n_phi;
+        st.phi0 = wrap_phi(K0 + pd.start + 4 * q, p.n_phi);
+        st.w_off = pd.w_off + 8u * (uint32_t)q;
+        q += st.nq; remaining -= st.nq;
+        return true;
+    };
+    auto issue = [&](const WideStage& st, const int b) {
+        char* zb = wsm + b * kWideStageBytes;
+        const int nchunks = kWideSpan / 4 + st.nq + 1;
+        int phi = wrap_phi(st.phi0 + 4 * lane, p.n_phi);
+        for (int c = lane; c < nchunks; c += 32) {
+            cp_async16(zb + ((c + (c >> 3)) << 4), st.row + phi);
+            phi += 128;
+            while (phi >= p.n_phi) phi -= p.n_phi;
+        }
+        char* wb = zb + kWideZChunks * 16;
+        const float* wsrc = p.weights + st.w_off;
+        for (int c = lane; c < 2 * st.nq; c += 32) cp_async16(wb + 16 * c, wsrc + 4 * c);
+        cp_async_commit();
+    };
+
+    uint64_t E[16], O[16];
 #pragma unroll
-            for (int u = 0; u < kPrefetchWide; u++) {
-                const int q = threadIdx.x + u * kThreads;
-                if (q < nxt.nq) pf[u] = quad_load(row_n, row_s, wrap_phi(nxt.phi4 + 4 * q, p.n_phi));
-            }
-            for (int q = threadIdx.x; q < (nxt.nt >> 2); q += kThreads) cp_async16(ws_n + 4 * q, p.weights + (size_t)nxt.w_off + 4 * q);
-        }
-        // ---- compute this warp's share of the taps of the current stage --------------------------------
-        {
-            const int chunk_taps = (((cur.nt >> 2) + S - 1) >> s_log2) << 2;
-            const int e_lo = s * chunk_taps;
-            const int e_hi = min(cur.nt, e_lo + chunk_taps);
-            conv_taps(acc, zs, ws, (uint32_t)cur.delta + lane_pair0, e_lo, e_hi);
-        }
-        // ---- commit the prefetched stage to the other buffer ---------------------------------------------
-        if (more) {
-#pragma unroll
-            for (int u = 0; u < kPrefetchWide; u++) {
-                const int q = threadIdx.x + u * kThreads;
-                if (q < nxt.nq) quad_store(zs_n, q, pf[u]);
-            }
-            cp_async_wait_all();
-        }
-        __syncthreads();
-        cur = nxt; buf ^= 1;
+    for (int m = 0; m < 16; m++) { E[m] = 0ull; O[m] = 0ull; }
+
+    WideStage cur, nxt;
+    bool have = next_stage(cur);
+    int b = 0;
+    if (have) issue(cur, 0);
+    while (have) {
+        const bool more = next_stage(nxt);
+        if (more) { issue(nxt, b ^ 1); cp_async_wait_group<1>(); } else { cp_async_wait_group<0>(); }
+        __syncwarp();
+        const char* zb = wsm + b * kWideStageBytes;
+        eo_taps(E, O, zb + lane * 144, reinterpret_cast<const ulonglong2*>(zb + kWideZChunks * 16), cur.nq);
+        __syncwarp();                                          // buffer b is free for the stage after next
+        cur = nxt; have = more; b ^= 1;
     }
 
-    // ---- epilogue -----------------------------------------------------------------------------------------
-    const int i = it.i0, i_s = p.n_theta - 1 - i;
+    // ---- epilogue: fold the two halves, sum the S splits in a fixed order, store float4 -----------------
+    float v[kWideP];
+#pragma unroll
+    for (int m = 0; m < 16; m++) {
+        float a0, a1, b0, b1;
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(E[m]));
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(b0), "=f"(b1) : "l"(O[m]));
+        v[2 * m] = a0 + a1; v[2 * m + 1] = b0 + b1;
+    }
+    float* orow = out + (size_t)i * p.n_phi;
     if (S == 1) {
-        store_outputs(p, out, i, it.k0 + (int)lane_pair0, acc);
-    } else {
-        // fixed-order sum of the S tap splits through shared memory (all stage buffers are free now)
-        __syncthreads();
-        uint64_t* red = reinterpret_cast<uint64_t*>(smem);
+        const int phi = K0 + lane * kWideP;
 #pragma unroll
-        for (int q = 0; q < kP; q++) red[(warp * kP + q) * 32 + lane] = acc[q];
+        for (int g = 0; g < kWideP / 4; g++)
+            if (phi + 4 * g < p.n_phi)
+                *reinterpret_cast<float4*>(orow + phi + 4 * g) = make_float4(v[4 * g], v[4 * g + 1], v[4 * g + 2], v[4 * g + 3]);
+    } else {
+        __syncthreads();                                       // every warp is done with its stage buffers
+        float* red = reinterpret_cast<float*>(smem);           // [warp][p][lane]
+#pragma unroll
+        for (int pp = 0; pp < kWideP; pp++) red[(warp * kWideP + pp) * 32 + lane] = v[pp];
         __syncthreads();
-        const int per = kP / S;
-        for (int q = s * per; q < (s + 1) * per; q++) {
-            float n = 0.f, so = 0.f;
-            for (int s2 = 0; s2 < S; s2++) {
-                const uint64_t v = red[((s2 * F + f) * kP + q) * 32 + lane];
-                float a, b;
-                asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
-                n += a; so += b;
+        const int per = (kWideP / 4) / S;                      // float4 groups of this lane's 32 outputs per split
+        for (int g = s * per; g < (s + 1) * per; g++) {
+            float o[4];
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                float sum = 0.f;
+                for (int s2 = 0; s2 < S; s2++) sum += red[((s2 * F + f) * kWideP + 4 * g + x) * 32 + lane];
+                o[x] = sum;
             }
-            const int phi = it.k0 + (int)lane_pair0 + q;
-            if (phi < p.n_phi) {
-                out[(size_t)i * p.n_phi + phi] = n;
-                if (i_s != i) out[(size_t)i_s * p.n_phi + phi] = so;
-            }
+            const int phi = K0 + lane * kWideP + 4 * g;
+            if (phi < p.n_phi) *reinterpret_cast<float4*>(orow + phi) = make_float4(o[0], o[1], o[2], o[3]);
         }
     }
 }

@@ -74,10 +74,8 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     s.R = (int)s.a_r.size() - 1;
     const int W = 2 * s.R + 1;
 
-    // ---- pair descriptors for the northern rings; work counters over ALL rings ------------------
+    // ---- windows of the northern ring pairs; work counters over ALL rings --------------------------
     s.pairs.assign((size_t)s.n_north * W, PairDesc{0u, 0, 0, -1});
-    unsigned long long w_off = 0;
-    std::vector<unsigned long long> ring_slots(s.n_north, 0);  // stored taps per output phi
     for (int i = 0; i < n_theta; i++) {
         for (int r = -s.R; r <= s.R; r++) {
             int j = i + r;
@@ -87,85 +85,131 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             unsigned long long taps = (D == n_phi) ? (unsigned long long)n_phi : (unsigned long long)(2 * D + 1);
             s.weights += taps;
             s.pair_evals += taps * (unsigned long long)n_phi;
-            if (i < s.n_north) {
-                PairDesc& p = s.pairs[(size_t)i * W + (r + s.R)];
-                p.half = D;
-                if (D == n_phi) { p.start = -(n_phi / 2); p.ntaps = n_phi; }
-                else { p.start = -(D + (D & 1)); p.ntaps = ((D - p.start + 1) + 3) & ~3; }
-                if (w_off + (unsigned long long)p.ntaps > 0xFFFFFFF0ull) return 4;
-                p.w_off = (uint32_t)w_off;
-                w_off += (unsigned long long)p.ntaps;
-                ring_slots[i] += (unsigned long long)p.ntaps;
-            }
+            if (i < s.n_north) s.pairs[(size_t)i * W + (r + s.R)].half = D;
         }
     }
-    s.weight_slots = w_off;
-
-    // ring-contiguous weight blocks (rows r = -R..R of one ring are stored back to back)
-    s.ring_w_off.assign(s.n_north, 0u); s.ring_slots.assign(s.n_north, 0u);
-    for (int i = 0; i < s.n_north; i++) {
-        bool first = true;
-        for (int r = 0; r < W; r++) {
-            const PairDesc& p = s.pairs[(size_t)i * W + r];
-            if (p.ntaps == 0) continue;
-            if (first) { s.ring_w_off[i] = p.w_off; first = false; }
-        }
-        s.ring_slots[i] = (uint32_t)ring_slots[i];
-    }
-
-    // ---- generator work units: one warp writes up to kGenUnitTaps taps of one ring pair -----------
-    for (int i = 0; i < s.n_north; i++)
-        for (int r = 0; r < W; r++) {
-            const PairDesc& p = s.pairs[(size_t)i * W + r];
-            const int j = i + r - s.R;
-            for (int e0 = 0; e0 < p.ntaps; e0 += kGenUnitTaps) {
-                GenUnit g;
-                g.w_base = p.w_off + (uint32_t)e0; g.d0 = p.start + e0;
-                g.count = std::min(kGenUnitTaps, p.ntaps - e0); g.half = p.half;
-                g.a = s.a_r[std::abs(r - s.R)]; g.b = s.sin_t[i] * s.sin_t[j]; g.area = s.area[j];
-                s.gen_units.push_back(g);
-            }
-        }
+    // stored tap range of a pair in the NARROW layout: start even, ntaps a multiple of 4
+    auto narrow_range = [&](int D, int& start, int& ntaps) {
+        if (D == n_phi) { start = -(n_phi / 2); ntaps = n_phi; }
+        else { start = -(D + (D & 1)); ntaps = ((D - start + 1) + 3) & ~3; }
+    };
+    // ... and in the WIDE (even/odd) layout: start a multiple of 4; T steps, T even, so that the odd
+    // outputs' pairs (w[2t-1], w[2t]) reach the last tap: 2T - 2 >= e_max
+    auto wide_range = [&](int D, int& start, int& ntaps) {
+        const int dmin = (D == n_phi) ? -(n_phi / 2) : -D;
+        const int dmax = (D == n_phi) ? n_phi / 2 - 1 : D;
+        start = -(((-dmin) + 3) & ~3);
+        const int e_max = dmax - start;
+        int T = (e_max + 1) / 2 + 1;
+        T = (T + 1) & ~1;
+        ntaps = 2 * T;
+    };
 
     // ---- ring classes -----------------------------------------------------------------------------
     // NARROW rings: every stored window lies inside [-kHaloNarrow, kHaloNarrow).  Windows widen
     // towards the pole, so the narrow rings are the band [first_narrow, n_north) next to the equator.
-    int f_cap = 0;                                            // largest useful F for this n_phi
-    while (f_cap < 3 && (kWarpSpan << f_cap) < n_phi) f_cap++;
     auto ring_is_narrow = [&](int i) {
         for (int r = 0; r < W; r++) {
             const PairDesc& p = s.pairs[(size_t)i * W + r];
-            if (p.ntaps == 0) continue;
-            if (p.half == n_phi || p.start < -kHaloNarrow || p.start + p.ntaps > kHaloNarrow) return false;
+            if (p.half < 0) continue;
+            if (p.half == n_phi) return false;
+            int start, ntaps;
+            narrow_range(p.half, start, ntaps);
+            if (start < -kHaloNarrow || start + ntaps > kHaloNarrow) return false;
         }
         return true;
     };
     s.first_narrow = s.n_north;
     while (s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
-    unsigned long long wslot = 0;
-    for (int i = s.first_narrow; i < s.n_north; i++) wslot = std::max<unsigned long long>(wslot, ring_slots[i]);
-    s.narrow_wslot = (int)((wslot + 3) & ~3ull);
+    {
+        unsigned long long wslot = 0;
+        for (int i = s.first_narrow; i < s.n_north; i++) {
+            unsigned long long slots = 0;
+            for (int r = 0; r < W; r++) {
+                const PairDesc& p = s.pairs[(size_t)i * W + r];
+                if (p.half < 0) continue;
+                int start, ntaps;
+                narrow_range(p.half, start, ntaps);
+                slots += (unsigned long long)ntaps;
+            }
+            wslot = std::max(wslot, slots);
+        }
+        s.narrow_wslot = (int)((wslot + 3) & ~3ull);
+    }
+    int nf_cap = 0;                                           // largest useful F of the narrow tiles
+    while (nf_cap < 3 && (kWarpSpan << nf_cap) < n_phi) nf_cap++;
     s.narrow_f_log2 = -1;
-    for (int fl = f_cap; fl >= 0; fl--)
+    for (int fl = nf_cap; fl >= 0; fl--)
         if (narrow_smem_bytes(fl, s.R, s.narrow_wslot) <= (size_t)kSmemBudget) { s.narrow_f_log2 = fl; break; }
     if (s.narrow_f_log2 < 0 || s.n_north - s.first_narrow < 1) { s.first_narrow = s.n_north; s.narrow_f_log2 = 0; }
 
+    // ---- weight layout ------------------------------------------------------------------------------
+    unsigned long long w_off = 0;
+    std::vector<unsigned long long> ring_slots(s.n_north, 0);  // stored taps per output phi
+    s.ring_w_off.assign(s.n_north, 0u); s.ring_slots.assign(s.n_north, 0u);
+    for (int i = 0; i < s.n_north; i++) {
+        const bool wide = i < s.first_narrow;
+        bool first = true;
+        for (int r = 0; r < W; r++) {
+            PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (p.half < 0) continue;
+            if (wide) wide_range(p.half, p.start, p.ntaps); else narrow_range(p.half, p.start, p.ntaps);
+            const unsigned long long floats = wide ? 2ull * p.ntaps : (unsigned long long)p.ntaps;
+            if (w_off + floats > 0xFFFFFFF0ull) return 4;
+            p.w_off = (uint32_t)w_off;
+            if (first) { s.ring_w_off[i] = p.w_off; first = false; }   // ring-contiguous weight block
+            w_off += floats;
+            ring_slots[i] += (unsigned long long)p.ntaps;
+        }
+        s.ring_slots[i] = (uint32_t)ring_slots[i];
+    }
+    s.weight_slots = w_off;
+
+    // ---- generator work units: one warp writes up to kGenUnitTaps taps (steps) of one ring pair -----
+    for (int i = 0; i < s.n_north; i++) {
+        const bool wide = i < s.first_narrow;
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            const int j = i + r - s.R;
+            const int n = wide ? p.ntaps / 2 : p.ntaps;          // steps or taps
+            for (int e0 = 0; e0 < n; e0 += kGenUnitTaps) {
+                GenUnit g;
+                g.w_base = p.w_off + (uint32_t)(wide ? 4 * e0 : e0); g.d0 = p.start + (wide ? 2 * e0 : e0);
+                g.count = std::min(kGenUnitTaps, n - e0); g.half = p.half;
+                g.a = s.a_r[std::abs(r - s.R)]; g.b = s.sin_t[i] * s.sin_t[j]; g.area = s.area[j];
+                g.eo = wide ? 1 : 0; g.pad_ = 0;
+                s.gen_units.push_back(g);
+            }
+        }
+    }
+
     // ---- work items, heaviest first (H1: polar imbalance) -------------------------------------------
     unsigned long long total = 0;
-    for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi;
+    for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi * (2 * i + 1 == n_theta ? 1ull : 2ull);
     const double c_max = (double)total / (double)sm_count / 8.0;   // no item above 1/8 of an SM's share, if possible
     struct Tmp { Item it; double cost; };
     std::vector<Tmp> tmp;
     size_t smem = 0;
-    // WIDE: (ring, phi tile of 512 F), F <= 4
-    for (int i = 0; i < s.first_narrow; i++) {
-        int fl = std::min(f_cap, 2);
-        while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWarpSpan << fl) > c_max) fl--;
-        const int L = kWarpSpan << fl;
-        smem = std::max(smem, wide_smem_bytes(fl, s.R));
-        for (int k0 = 0; k0 < n_phi; k0 += L) {
-            tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kWide, 1}, (double)ring_slots[i] * (double)L + 4000.0});
-            s.fma_slots += 2ull * ring_slots[i] * (unsigned long long)L;      // x2: both mirror rings
+    // WIDE: (ring of either hemisphere, phi tile of F sub-tiles of kWideSpan outputs); S = 8/F tap splits
+    if (s.first_narrow > 0) {
+        smem = std::max(smem, wide_smem_bytes(s.R));
+        int wf_cap = 0;
+        while (wf_cap < 3 && (kWideSpan << wf_cap) < n_phi) wf_cap++;
+        for (int i = 0; i < s.first_narrow; i++) {
+            int fl = wf_cap;
+            while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWideSpan << fl) > c_max) fl--;
+            const int L = kWideSpan << fl;
+            const int i_s = n_theta - 1 - i;
+            for (int k0 = 0; k0 < n_phi; k0 += L) {
+                const int valid = std::min(L, n_phi - k0);
+                const double cost = (double)ring_slots[i] * (double)valid + 4000.0;
+                tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
+                s.fma_slots += ring_slots[i] * (unsigned long long)L;
+                if (i_s != i) {
+                    tmp.push_back(Tmp{Item{i_s, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
+                    s.fma_slots += ring_slots[i] * (unsigned long long)L;
+                }
+            }
         }
     }
     // NARROW: (band of B rings, phi tile of 512 F); S = 8/F rings advance together
@@ -176,11 +220,11 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         int i = s.first_narrow;
         while (i < s.n_north) {
             double c = 0.0; int b = 0;
-            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += (double)ring_slots[i + b] * (double)L; b++; }
+            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += 2.0 * (double)ring_slots[i + b] * (double)L; b++; }
             b = std::min((b + S - 1) / S * S, s.n_north - i);
             if (s.n_north - (i + b) < b_min / 2) b = s.n_north - i;     // do not leave a tiny tail band
             c = 0.0;
-            for (int q = 0; q < b; q++) c += (double)ring_slots[i + q] * (double)L;
+            for (int q = 0; q < b; q++) c += 2.0 * (double)ring_slots[i + q] * (double)L;
             for (int k0 = 0; k0 < n_phi; k0 += L) {
                 tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, b}, c + 4000.0});
                 for (int q = 0; q < b; q++) s.fma_slots += 2ull * ring_slots[i + q] * (unsigned long long)L;
@@ -189,17 +233,17 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         }
     }
     s.smem_bytes = smem;
+    for (const Tmp& t : tmp)
+        if (t.it.kind == kWide) s.fma_slots_wide += ring_slots[std::min(t.it.i0, n_theta - 1 - t.it.i0)] * (unsigned long long)(kWideSpan << t.it.f_log2);
     std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
     s.items.reserve(tmp.size());
     for (auto& t : tmp) s.items.push_back(t.it);
     return 0;
 }
 
-size_t wide_smem_bytes(int f_log2, int R) {
-    const int L = kWarpSpan << f_log2, TB = tap_block(f_log2);
-    const size_t cap_pairs = (size_t)((L + TB + 8 + 15) & ~15);
-    const size_t stage = 2 * (cap_pairs * 8 + (size_t)TB * 4) + (size_t)(2 * R + 1) * sizeof(PairDesc);
-    const size_t red = (size_t)kWarps * kP * 32 * 8;
+size_t wide_smem_bytes(int R) {
+    const size_t stage = (size_t)kWarps * 2 * kWideStageBytes + (size_t)(2 * R + 1) * sizeof(PairDesc);
+    const size_t red = (size_t)kWarps * kWideSpan * 4;
     return stage > red ? stage : red;
 }
 
