@@ -27,8 +27,8 @@ constexpr int kSmemBudget = 220 * 1024;
 // ring's taps through a private, double-buffered shared-memory stage of kWideStage tap pairs.
 constexpr int kWideP = 32;                          // outputs per lane
 constexpr int kWideSpan = 32 * kWideP;              // 1024 outputs per warp
-constexpr int kWideStage = 128;                     // tap pairs ("steps") per stage; even
-constexpr int kWideZChunks = 368;                   // 16-byte chunks of a stage's input window: (1024 + 2*128 + 4)/4 = 321
+constexpr int kWideStage = 256;                     // tap pairs ("steps") per stage; even
+constexpr int kWideZChunks = 440;                   // 16-byte chunks of a stage's input window: (1024 + 2*128 + 4)/4 = 321
                                                     //   logical chunks, one pad chunk after every 8 (lane stride 9 chunks)
 constexpr int kWideWBytes = (kWideStage + 4) * 16;  // weights of a stage: 16 bytes per step (+ prefetch slack)
 constexpr int kWideStageBytes = kWideZChunks * 16 + kWideWBytes;

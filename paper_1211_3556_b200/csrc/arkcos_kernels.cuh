@@ -232,41 +232,46 @@ __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.w
 
 constexpr int kZRing = 10;                // register window: 10 chunks = 20 input pairs (17 live + prefetch)
 
+// 16-byte shared-memory load that the compiler may not sink, hoist or drop: the loads below are
+// software prefetches issued one double step ahead of their first use.
+__device__ __forceinline__ void lds128(uint64_t& a, uint64_t& b, const uint32_t addr) {
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
+}
+
 // One double step (4 taps) at window phase PH.  Live chunks q .. q+8 sit in ring slots (PH + c) % 10;
-// chunk q+9 is fetched into the slot chunk q-1 has just left, weights of double step q+1 into wn.
+// chunk q+9 is fetched into the slot chunk q-1 has just left, the weights of double step q+1 into the
+// other half of the weight double buffer.
 template <int PH>
 __device__ __forceinline__ void eo_dstep(uint64_t (&E)[16], uint64_t (&O)[16], uint64_t (&z)[2 * kZRing],
-                                         ulonglong2 (&w)[2], const char* __restrict__ zlane,
-                                         const ulonglong2* __restrict__ ws, const int q) {
+                                         uint64_t (&w)[2][4], const uint32_t zlane, const uint32_t ws, const int q) {
+    constexpr int B = PH & 1;
     const int u = q + 9;
-    const ulonglong2 nz = *reinterpret_cast<const ulonglong2*>(zlane + ((u + (u >> 3)) << 4));
-    const ulonglong2 wn0 = ws[2 * q + 2], wn1 = ws[2 * q + 3];
+    lds128(z[(2 * (PH + 9)) % (2 * kZRing)], z[(2 * (PH + 9) + 1) % (2 * kZRing)], zlane + (uint32_t)((u + (u >> 3)) << 4));
+    lds128(w[B ^ 1][0], w[B ^ 1][1], ws + (uint32_t)(32 * q + 32));
+    lds128(w[B ^ 1][2], w[B ^ 1][3], ws + (uint32_t)(32 * q + 48));
 #pragma unroll
     for (int m = 0; m < 16; m++) {
-        ffma2p(E[m], z[(2 * PH + m) % (2 * kZRing)], w[0].x);
-        ffma2p(O[m], z[(2 * PH + m) % (2 * kZRing)], w[0].y);
+        ffma2p(E[m], z[(2 * PH + m) % (2 * kZRing)], w[B][0]);
+        ffma2p(O[m], z[(2 * PH + m) % (2 * kZRing)], w[B][1]);
     }
 #pragma unroll
     for (int m = 0; m < 16; m++) {
-        ffma2p(E[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[1].x);
-        ffma2p(O[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[1].y);
+        ffma2p(E[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[B][2]);
+        ffma2p(O[m], z[(2 * PH + 1 + m) % (2 * kZRing)], w[B][3]);
     }
-    z[(2 * (PH + 9)) % (2 * kZRing)] = nz.x;
-    z[(2 * (PH + 9) + 1) % (2 * kZRing)] = nz.y;
-    w[0] = wn0; w[1] = wn1;
 }
 
 // E[m] += sum_t Z[m+t] * ws[t].x,  O[m] += sum_t Z[m+t] * ws[t].y  over t = 0 .. 2 nq - 1
-__device__ __forceinline__ void eo_taps(uint64_t (&E)[16], uint64_t (&O)[16], const char* __restrict__ zlane,
-                                        const ulonglong2* __restrict__ ws, const int nq) {
+// zlane / ws: shared-memory addresses of the lane's first chunk and of the stage's weights.
+__device__ __forceinline__ void eo_taps(uint64_t (&E)[16], uint64_t (&O)[16], const uint32_t zlane, const uint32_t ws,
+                                        const int nq) {
     uint64_t z[2 * kZRing];
 #pragma unroll
-    for (int c = 0; c < 9; c++) {
-        const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(zlane + ((c + (c >> 3)) << 4));
-        z[2 * c] = v.x; z[2 * c + 1] = v.y;
-    }
+    for (int c = 0; c < 9; c++) lds128(z[2 * c], z[2 * c + 1], zlane + (uint32_t)((c + (c >> 3)) << 4));
     z[18] = 0ull; z[19] = 0ull;
-    ulonglong2 w[2] = {ws[0], ws[1]};
+    uint64_t w[2][4];
+    lds128(w[0][0], w[0][1], ws);
+    lds128(w[0][2], w[0][3], ws + 16);
     int q = 0;
     for (;;) {
         eo_dstep<0>(E, O, z, w, zlane, ws, q); if (++q == nq) break;
@@ -298,6 +303,7 @@ __device__ void conv_wide(const ConvParams& p, const Item& it, uint4* smem, cons
     const bool mirrored = 2 * i >= p.n_theta;                  // southern ring: weights of its mirror pair
     const int i_n = mirrored ? p.n_theta - 1 - i : i;
     char* wsm = reinterpret_cast<char*>(smem) + (size_t)warp * 2 * kWideStageBytes;
+    const uint32_t wsm_addr = (uint32_t)__cvta_generic_to_shared(wsm);
     PairDesc* spd = reinterpret_cast<PairDesc*>(reinterpret_cast<char*>(smem) + (size_t)kWarps * 2 * kWideStageBytes);
     for (int r = threadIdx.x; r < W; r += kThreads) spd[r] = p.pairs[(size_t)i_n * W + r];
     __syncthreads();
@@ -326,14 +332,22 @@ __device__ void conv_wide(const ConvParams& p, const Item& it, uint4* smem, cons
         q += st.nq; remaining -= st.nq;
         return true;
     };
+    // lane-constant parts of the stage fill: chunk c = lane + 32 n sits at physical chunk
+    // (lane + (lane >> 3)) + 36 n, its input at phi0 + 4 lane + 128 n (mod n_phi)
+    const int lane_phi = (4 * lane) % p.n_phi, phi_step = 128 % p.n_phi;
+    const int lane_dst = (lane + (lane >> 3)) << 4;
     auto issue = [&](const WideStage& st, const int b) {
         char* zb = wsm + b * kWideStageBytes;
         const int nchunks = kWideSpan / 4 + st.nq + 1;
-        int phi = wrap_phi(st.phi0 + 4 * lane, p.n_phi);
+        int phi = st.phi0 + lane_phi;
+        if (phi >= p.n_phi) phi -= p.n_phi;
+        char* dst = zb + lane_dst;
+#pragma unroll 4
         for (int c = lane; c < nchunks; c += 32) {
-            cp_async16(zb + ((c + (c >> 3)) << 4), st.row + phi);
-            phi += 128;
-            while (phi >= p.n_phi) phi -= p.n_phi;
+            cp_async16(dst, st.row + phi);
+            dst += 36 * 16;
+            phi += phi_step;
+            if (phi >= p.n_phi) phi -= p.n_phi;
         }
         char* wb = zb + kWideZChunks * 16;
         const float* wsrc = p.weights + st.w_off;
@@ -353,8 +367,8 @@ __device__ void conv_wide(const ConvParams& p, const Item& it, uint4* smem, cons
         const bool more = next_stage(nxt);
         if (more) { issue(nxt, b ^ 1); cp_async_wait_group<1>(); } else { cp_async_wait_group<0>(); }
         __syncwarp();
-        const char* zb = wsm + b * kWideStageBytes;
-        eo_taps(E, O, zb + lane * 144, reinterpret_cast<const ulonglong2*>(zb + kWideZChunks * 16), cur.nq);
+        const uint32_t zb = wsm_addr + (uint32_t)(b * kWideStageBytes);
+        eo_taps(E, O, zb + (uint32_t)(lane * 144), zb + (uint32_t)(kWideZChunks * 16), cur.nq);
         __syncwarp();                                          // buffer b is free for the stage after next
         cur = nxt; have = more; b ^= 1;
     }
