@@ -184,6 +184,7 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
             if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); st = ARKCOS_ENOMEM; break; }
             if (!cuda_ok(e, "cudaMalloc(weights)")) { st = ARKCOS_ECUDA; break; }
             pl->device_bytes += bytes;
+            if (!cuda_ok(cudaMemset(pl->d_weights, 0, bytes), "cudaMemset(weights)")) { st = ARKCOS_ECUDA; break; }
         }
         // launch configuration
         const size_t smem = s.smem_bytes;
@@ -319,15 +320,14 @@ arkcos_status arkcos_plan_pair_weights(const arkcos_plan* pl, int i, int j, floa
     CU(cudaDeviceSynchronize());
     int dmax = pd->half == s.n_phi ? s.n_phi / 2 : pd->half;
     int cnt = dmax + 1 < cap ? dmax + 1 : cap;
-    const bool eo = in_ < s.first_narrow;                     // wide ring: even/odd step layout (PairDesc)
-    const size_t floats = eo ? 2 * (size_t)pd->ntaps : (size_t)pd->ntaps;
+    const size_t floats = (size_t)pd->ntaps;
     std::vector<float> all(floats);
     CU(cudaMemcpy(all.data(), pl->d_weights + pd->w_off, sizeof(float) * floats, cudaMemcpyDeviceToHost));
     for (int d = 0; d < cnt; d++) {
         // tap +d is stored at e = d - start, except d = n_phi/2 of a whole ring, stored as d = -n_phi/2
         int e = d - pd->start;
         if (pd->half == s.n_phi && d == s.n_phi / 2) e = -d - pd->start;
-        h_w[d] = eo ? all[4 * (size_t)(e >> 1) + (e & 1)] : all[e];
+        h_w[d] = all[e];
     }
     *n = cnt;
     return ARKCOS_OK;

@@ -13,36 +13,45 @@
 namespace arkcos {
 
 // ---- tiling constants of the convolution kernel ---------------------
-constexpr int kP = 16;                 // outputs per thread in phi (register-blocked sliding window)
-constexpr int kWarpSpan = 32 * kP;     // 512 contiguous phi outputs per warp
+// A lane owns kLaneP consecutive phi outputs of one ring in registers; a warp owns kWarpSpan.  The hot
+// loops are plain FP32 FFMA with the (warp-uniform) weight as the re-used operand: measured on B200,
+// that form issues at 124 of the 128 FMA/clk/SM, against 94 for the packed FFMA2 form.
+constexpr int kLaneP = 32;             // outputs per lane in phi
+constexpr int kWarpSpan = 32 * kLaneP; // 1024 contiguous phi outputs per warp
 constexpr int kWarps = 8;              // warps per CTA
 constexpr int kThreads = 32 * kWarps;
 constexpr int kHaloNarrow = 32;        // narrow rings: every stored tap window lies inside [-32, 32)
-constexpr int kPrefetchNarrow = 5;     // ... for the next narrow pass (S new rows)
 constexpr int kGenUnitTaps = 1024;     // taps per weight-generator work unit (one warp)
 constexpr int kSmemBudget = 220 * 1024;
 
-// ---- WIDE items (windows of 64 .. n_phi taps): warp-autonomous even/odd-tap path -----------------
-// A warp owns kWideSpan contiguous outputs of ONE ring (32 per lane) and streams its share of the
-// ring's taps through a private, double-buffered shared-memory stage of kWideStage tap pairs.
-constexpr int kWideP = 32;                          // outputs per lane
-constexpr int kWideSpan = 32 * kWideP;              // 1024 outputs per warp
-constexpr int kWideStage = 256;                     // tap pairs ("steps") per stage; even
-constexpr int kWideZChunks = 440;                   // 16-byte chunks of a stage's input window: (1024 + 2*128 + 4)/4 = 321
-                                                    //   logical chunks, one pad chunk after every 8 (lane stride 9 chunks)
-constexpr int kWideWBytes = (kWideStage + 4) * 16;  // weights of a stage: 16 bytes per step (+ prefetch slack)
-constexpr int kWideStageBytes = kWideZChunks * 16 + kWideWBytes;
+// Shared-memory rows are stored in lane tiles: 8 chunks of 16 bytes (the kLaneP floats one lane owns)
+// followed by one pad chunk, so that the 16-byte / 8-byte loads of the 32 lanes of a warp (lane stride
+// 144 bytes) are bank-conflict free.  Logical 16-byte chunk c sits at physical chunk c + (c >> 3).
+constexpr int kTileBytes = 144;
+
+// ---- NARROW items: band marching -----------------------------------------------------------------
+// Row slot = left halo tile + F * 32 own tiles + right halo tile + one spare tile (software prefetch
+// of the sliding window reads at most one tile past the right halo).
+ARKCOS_HD constexpr int narrow_slot_bytes(int f_log2) { return ((32 << f_log2) + 3) * kTileBytes; }
+
+// ---- WIDE items (windows of 64 .. n_phi taps): warp-autonomous path ------------------------------
+// A warp owns kWarpSpan contiguous outputs of ONE ring and streams its share of the ring's taps through
+// a private, double-buffered shared-memory stage of up to kWideStage taps.
+constexpr int kWideStage = 512;                     // taps per stage; multiple of 4
+constexpr int kWideZChunks = (kWarpSpan + kWideStage) / 4 + 8;          // logical chunks of a stage's input window (+ prefetch slack)
+constexpr int kWideZBytes = (kWideZChunks + kWideZChunks / 8 + 1) * 16; // ... in the padded tile layout
+constexpr int kWideWBytes = (kWideStage + 8) * 4;   // weights of a stage (+ prefetch slack)
+constexpr int kWideStageBytes = kWideZBytes + kWideWBytes;
 
 // One (north output ring i, input ring j = i + r) pair.  The southern mirror pair
-// (n_theta-1-i, n_theta-1-j) has identical weights.
-//   NARROW rings: `ntaps` FP32 weights w[e], tap e <-> dphi index d = start + e.
-//   WIDE rings:   ntaps/2 steps of 4 floats (K(d), K(d+1), K(d-1), K(d)), d = start + 2t: the weight
-//                 pairs of the even and of the odd outputs for the aligned input pair (x[d], x[d+1]);
-//                 2*ntaps floats in all; start is a multiple of 4.
+// (n_theta-1-i, n_theta-1-j) has identical weights.  `ntaps` FP32 weights w[e], tap e <-> dphi index
+// d = start + e; zero outside the window.
+//   NARROW rings: start and ntaps even (8-byte steps), window inside [-32, 32).
+//   WIDE rings:   start and ntaps multiples of 4 (16-byte steps).
 struct PairDesc {
-    uint32_t w_off;   // offset, in floats, of the stored weights; multiple of 4
-    int32_t start;    // dphi index d of stored tap 0 (even, <= 0)
-    int32_t ntaps;    // stored taps, multiple of 4; 0 = nothing to do
+    uint32_t w_off;   // offset, in floats, of the stored weights; even (narrow) / multiple of 4 (wide)
+    int32_t start;    // dphi index d of stored tap 0 (<= 0)
+    int32_t ntaps;    // stored taps; 0 = nothing to do
     int32_t half;     // D (taps -D..D inside theta_cut); n_phi = whole ring; -1 = empty
 };
 
@@ -53,14 +62,13 @@ struct Item {
     int32_t i0;       // kWide: the output ring (either hemisphere).  kNarrow: first NORTHERN output ring
                       //   (the CTA also produces the mirror rings)
     int32_t k0;       // first output phi of the tile
-    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles (kWideSpan outputs wide, 512 narrow); S = kWarps / F
+    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles of kWarpSpan outputs; S = kWarps / F
     int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings, S rings per pass
-    int32_t nrings;
+    int32_t nrings;   // kNarrow: rings of the band; negative = the band is the southern mirror of
+                      //   northern rings [i0, i0 - nrings)
 };
 
-// Work unit of the weight generator (one warp) for one ring pair.
-//   eo == 0: `count` taps d0, d0+1, ...            -> count floats
-//   eo == 1: `count` steps d = d0, d0+2, ...       -> 4 count floats (K(d), K(d+1), K(d-1), K(d))
+// Work unit of the weight generator (one warp) for one ring pair: `count` taps d0, d0+1, ...
 struct GenUnit {
     uint32_t w_base;  // destination offset in the weight buffer
     int32_t d0;       // first dphi index
@@ -69,8 +77,7 @@ struct GenUnit {
     double a;         // sin^2((t_i - t_j)/2)
     double b;         // sin t_i sin t_j
     double area;      // A_j
-    int32_t eo;       // layout, see above
-    int32_t pad_;
+    int32_t pad_[2];
 };
 
 // Host-side result of step S1 (the ring-pair scheduler).  FP64 throughout.
@@ -86,7 +93,7 @@ struct Schedule {
     std::vector<double> s2;                 // [n_phi/2+1] sin^2(d dphi / 2)
     std::vector<PairDesc> pairs;            // [n_north][2R+1]
     std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
-    std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows)
+    std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows, padded to 4)
     std::vector<Item> items;                // cost-sorted, heaviest first
     std::vector<GenUnit> gen_units;
     int first_narrow = 0;                   // rings [first_narrow, n_north) use the narrow kernel path

@@ -88,21 +88,17 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             if (i < s.n_north) s.pairs[(size_t)i * W + (r + s.R)].half = D;
         }
     }
-    // stored tap range of a pair in the NARROW layout: start even, ntaps a multiple of 4
+    // stored tap range of a pair in the NARROW layout: start and ntaps even (8-byte steps)
     auto narrow_range = [&](int D, int& start, int& ntaps) {
         if (D == n_phi) { start = -(n_phi / 2); ntaps = n_phi; }
-        else { start = -(D + (D & 1)); ntaps = ((D - start + 1) + 3) & ~3; }
+        else { start = -(D + (D & 1)); ntaps = ((D - start + 1) + 1) & ~1; }
     };
-    // ... and in the WIDE (even/odd) layout: start a multiple of 4; T steps, T even, so that the odd
-    // outputs' pairs (w[2t-1], w[2t]) reach the last tap: 2T - 2 >= e_max
+    // ... and in the WIDE layout: start and ntaps multiples of 4 (16-byte steps)
     auto wide_range = [&](int D, int& start, int& ntaps) {
         const int dmin = (D == n_phi) ? -(n_phi / 2) : -D;
         const int dmax = (D == n_phi) ? n_phi / 2 - 1 : D;
         start = -(((-dmin) + 3) & ~3);
-        const int e_max = dmax - start;
-        int T = (e_max + 1) / 2 + 1;
-        T = (T + 1) & ~1;
-        ntaps = 2 * T;
+        ntaps = ((dmax - start + 1) + 3) & ~3;
     };
 
     // ---- ring classes -----------------------------------------------------------------------------
@@ -154,30 +150,30 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half < 0) continue;
             if (wide) wide_range(p.half, p.start, p.ntaps); else narrow_range(p.half, p.start, p.ntaps);
-            const unsigned long long floats = wide ? 2ull * p.ntaps : (unsigned long long)p.ntaps;
+            const unsigned long long floats = (unsigned long long)p.ntaps;
             if (w_off + floats > 0xFFFFFFF0ull) return 4;
             p.w_off = (uint32_t)w_off;
             if (first) { s.ring_w_off[i] = p.w_off; first = false; }   // ring-contiguous weight block
             w_off += floats;
             ring_slots[i] += (unsigned long long)p.ntaps;
         }
-        s.ring_slots[i] = (uint32_t)ring_slots[i];
+        w_off = (w_off + 3) & ~3ull;                                   // every ring's block is 16-byte aligned
+        s.ring_slots[i] = (uint32_t)((ring_slots[i] + 3) & ~3ull);
     }
     s.weight_slots = w_off;
 
     // ---- generator work units: one warp writes up to kGenUnitTaps taps (steps) of one ring pair -----
     for (int i = 0; i < s.n_north; i++) {
-        const bool wide = i < s.first_narrow;
         for (int r = 0; r < W; r++) {
             const PairDesc& p = s.pairs[(size_t)i * W + r];
             const int j = i + r - s.R;
-            const int n = wide ? p.ntaps / 2 : p.ntaps;          // steps or taps
+            const int n = p.ntaps;
             for (int e0 = 0; e0 < n; e0 += kGenUnitTaps) {
                 GenUnit g;
-                g.w_base = p.w_off + (uint32_t)(wide ? 4 * e0 : e0); g.d0 = p.start + (wide ? 2 * e0 : e0);
+                g.w_base = p.w_off + (uint32_t)e0; g.d0 = p.start + e0;
                 g.count = std::min(kGenUnitTaps, n - e0); g.half = p.half;
                 g.a = s.a_r[std::abs(r - s.R)]; g.b = s.sin_t[i] * s.sin_t[j]; g.area = s.area[j];
-                g.eo = wide ? 1 : 0; g.pad_ = 0;
+                g.pad_[0] = g.pad_[1] = 0;
                 s.gen_units.push_back(g);
             }
         }
@@ -190,29 +186,28 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     struct Tmp { Item it; double cost; };
     std::vector<Tmp> tmp;
     size_t smem = 0;
-    // WIDE: (ring of either hemisphere, phi tile of F sub-tiles of kWideSpan outputs); S = 8/F tap splits
+    // WIDE: (ring of either hemisphere, phi tile of F sub-tiles of kWarpSpan outputs); S = 8/F tap splits
     if (s.first_narrow > 0) {
         smem = std::max(smem, wide_smem_bytes(s.R));
         int wf_cap = 0;
-        while (wf_cap < 3 && (kWideSpan << wf_cap) < n_phi) wf_cap++;
+        while (wf_cap < 3 && (kWarpSpan << wf_cap) < n_phi) wf_cap++;
         for (int i = 0; i < s.first_narrow; i++) {
             int fl = wf_cap;
-            while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWideSpan << fl) > c_max) fl--;
-            const int L = kWideSpan << fl;
+            while (fl > 0 && (double)ring_slots[i] * (double)std::min(n_phi, kWarpSpan << fl) > c_max) fl--;
+            const int L = kWarpSpan << fl;
             const int i_s = n_theta - 1 - i;
             for (int k0 = 0; k0 < n_phi; k0 += L) {
                 const int valid = std::min(L, n_phi - k0);
                 const double cost = (double)ring_slots[i] * (double)valid + 4000.0;
-                tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
-                s.fma_slots += ring_slots[i] * (unsigned long long)L;
-                if (i_s != i) {
-                    tmp.push_back(Tmp{Item{i_s, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
+                for (int hemi = 0; hemi < (i_s != i ? 2 : 1); hemi++) {
+                    tmp.push_back(Tmp{Item{hemi ? i_s : i, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
                     s.fma_slots += ring_slots[i] * (unsigned long long)L;
+                    s.fma_slots_wide += ring_slots[i] * (unsigned long long)L;
                 }
             }
         }
     }
-    // NARROW: (band of B rings, phi tile of 512 F); S = 8/F rings advance together
+    // NARROW: (band of B rings of one hemisphere, phi tile of F * kWarpSpan outputs); S = 8/F rings advance together
     if (s.first_narrow < s.n_north) {
         const int fl = s.narrow_f_log2, S = kWarps >> fl, L = kWarpSpan << fl;
         smem = std::max(smem, narrow_smem_bytes(fl, s.R, s.narrow_wslot));
@@ -220,21 +215,25 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         int i = s.first_narrow;
         while (i < s.n_north) {
             double c = 0.0; int b = 0;
-            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += 2.0 * (double)ring_slots[i + b] * (double)L; b++; }
+            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += (double)ring_slots[i + b] * (double)L; b++; }
             b = std::min((b + S - 1) / S * S, s.n_north - i);
             if (s.n_north - (i + b) < b_min / 2) b = s.n_north - i;     // do not leave a tiny tail band
-            c = 0.0;
-            for (int q = 0; q < b; q++) c += 2.0 * (double)ring_slots[i + q] * (double)L;
-            for (int k0 = 0; k0 < n_phi; k0 += L) {
-                tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, b}, c + 4000.0});
-                for (int q = 0; q < b; q++) s.fma_slots += 2ull * ring_slots[i + q] * (unsigned long long)L;
+            // the southern mirror band leaves out a ring that is its own mirror (odd n_theta: the equator)
+            const int b_south = (2 * (i + b - 1) + 1 == n_theta) ? b - 1 : b;
+            for (int hemi = 0; hemi < 2; hemi++) {
+                const int nb = hemi ? b_south : b;
+                if (nb <= 0) continue;
+                c = 0.0;
+                for (int q = 0; q < nb; q++) c += (double)ring_slots[i + q] * (double)L;
+                for (int k0 = 0; k0 < n_phi; k0 += L) {
+                    tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, hemi ? -nb : nb}, c + 4000.0});
+                    for (int q = 0; q < nb; q++) s.fma_slots += ring_slots[i + q] * (unsigned long long)L;
+                }
             }
             i += b;
         }
     }
     s.smem_bytes = smem;
-    for (const Tmp& t : tmp)
-        if (t.it.kind == kWide) s.fma_slots_wide += ring_slots[std::min(t.it.i0, n_theta - 1 - t.it.i0)] * (unsigned long long)(kWideSpan << t.it.f_log2);
     std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
     s.items.reserve(tmp.size());
     for (auto& t : tmp) s.items.push_back(t.it);
@@ -243,14 +242,16 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
 
 size_t wide_smem_bytes(int R) {
     const size_t stage = (size_t)kWarps * 2 * kWideStageBytes + (size_t)(2 * R + 1) * sizeof(PairDesc);
-    const size_t red = (size_t)kWarps * kWideSpan * 4;
+    const size_t red = (size_t)kWarps * kWarpSpan * 4;
     return stage > red ? stage : red;
 }
 
+// (2R + 2S) row slots (the S rows of the next pass land in the slots the previous pass freed), two
+// buffers of S ring weight blocks and of S x (2R+1) pair descriptors
 size_t narrow_smem_bytes(int f_log2, int R, int wslot) {
     const int S = kWarps >> f_log2;
-    const size_t slot_pairs = (size_t)(kWarpSpan << f_log2) + 2 * kHaloNarrow;
-    return (size_t)(2 * R + S) * slot_pairs * 8 + 2ull * S * (size_t)wslot * 4 + 2ull * S * (2 * R + 1) * sizeof(PairDesc);
+    return (size_t)(2 * R + 2 * S) * (size_t)narrow_slot_bytes(f_log2) + 2ull * S * (size_t)wslot * 4 +
+           2ull * S * (2 * R + 1) * sizeof(PairDesc);
 }
 
 }  // namespace arkcos
