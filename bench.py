@@ -168,7 +168,8 @@ def workload_config(w: wl.Workload):
                 8e-6 * w.n_pix, "larger than L2, no flush needed" if 8 * w.n_pix > 126e6 else "input buffers rotated")}
 
 
-def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True):
+def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
+            only: str = "all"):
     import torch
     from paper_1211_3556_b200 import arkcos
 
@@ -177,7 +178,10 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     hbm_gbs, sm_max_mhz, peak_src = load_peaks()
     table = w.table()
     x32 = w.map_f32()
-    plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut)
+    # --only wide|narrow: the library's measurement hook launches one class of work items only (the
+    # output is then incomplete; used for per-class timing and ncu captures, never for the bench line)
+    flags = {"all": 0, "wide": arkcos.PLAN_ONLY_WIDE, "narrow": arkcos.PLAN_ONLY_NARROW}[only]
+    plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
     sh = stream.cuda_stream
@@ -298,6 +302,9 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=1 << 17, help="oracle sample per step of --impl reference")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="five-config report + cost-vs-theta_cut curve")
+    ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
+                    help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
+                         "prints a per-class line, not the bench line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = wl.by_name(args.workload)
@@ -314,6 +321,19 @@ def main():
     if args.sweep:
         if rank == 0:
             sweep(args)
+        return 0
+
+    if args.only != "all":
+        if rank == 0:
+            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only)
+            info = res["info"]
+            slots = int(info.fma_slots_wide) if args.only == "wide" else int(info.fma_slots) - int(info.fma_slots_wide)
+            peak = res["sm_count"] * FP32_LANES_PER_SM * res["sm_max_mhz"] * 1e6
+            print(json.dumps({"report": "class_only", "only": args.only, "workload": w.name, "items": int(info.n_items),
+                              "convolve_ms": res["conv_ms"], "fma_slots": slots,
+                              "issued_lane_frac": slots / (res["conv_ms"] * 1e-3) / peak, "clocks": res["clocks"]}), flush=True)
+        if dist is not None:
+            dist.destroy_process_group()
         return 0
 
     res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False)
