@@ -45,7 +45,11 @@ __device__ __forceinline__ float gen_weight(const GenParams& p, const GenUnit& g
 }
 
 __global__ void __launch_bounds__(kGenThreads) k_generate_weights(const GenParams p) {
+#ifndef ARKCOS_HOST_EMU
     extern __shared__ double s_table[];
+#else
+    double* s_table = reinterpret_cast<double*>(emu::g_smem);
+#endif
     const double* tab = p.table;
     if (p.table_in_smem) {
         for (int m = threadIdx.x; m < p.n_table; m += blockDim.x) s_table[m] = p.table[m];
@@ -91,6 +95,10 @@ struct ConvParams {
     long long map_stride;    // elements between consecutive maps of a batch
 };
 
+// ---- the PTX this file uses, in one place --------------------------------------------------------
+// (ARKCOS_HOST_EMU: tests/emu/ compiles this very file for the host to check the index logic of the
+//  kernels against the oracle without a GPU; the emulation replaces only these wrappers.)
+#ifndef ARKCOS_HOST_EMU
 __device__ __forceinline__ void cp_async16(const uint32_t smem_dst, const void* gmem_src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
 }
@@ -98,11 +106,6 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-__device__ __forceinline__ int wrap_phi(int phi, int n_phi) {   // phi may be any int; result in [0, n_phi)
-    int r = phi % n_phi;
-    return r < 0 ? r + n_phi : r;
-}
 
 // Shared-memory loads that the compiler may not sink, hoist or drop: they are software prefetches
 // issued one step ahead of their first use.
@@ -116,6 +119,29 @@ __device__ __forceinline__ void lds128i(float& a, float& b, float& c, float& d, 
 template <int OFF>
 __device__ __forceinline__ void lds64i(float& a, float& b, const uint32_t addr) {
     asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(a), "=f"(b) : "r"(addr), "n"(OFF));
+}
+#else
+__device__ __forceinline__ void cp_async16(const uint32_t smem_dst, const void* gmem_src) { emu::cp_async_enqueue(smem_dst, gmem_src); }
+__device__ __forceinline__ void cp_async_commit() { emu::cp_async_commit_group(); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { emu::cp_async_wait(N); }
+__device__ __forceinline__ void cp_async_wait_all() { emu::cp_async_wait(0); }
+__device__ __forceinline__ void lds128(float& a, float& b, float& c, float& d, const uint32_t addr) {
+    const float* q = reinterpret_cast<const float*>(emu::smem_at(addr, 16));
+    a = q[0]; b = q[1]; c = q[2]; d = q[3];
+}
+template <int OFF>
+__device__ __forceinline__ void lds128i(float& a, float& b, float& c, float& d, const uint32_t addr) { lds128(a, b, c, d, addr + (uint32_t)OFF); }
+template <int OFF>
+__device__ __forceinline__ void lds64i(float& a, float& b, const uint32_t addr) {
+    const float* q = reinterpret_cast<const float*>(emu::smem_at(addr + (uint32_t)OFF, 8));
+    a = q[0]; b = q[1];
+}
+#endif
+
+__device__ __forceinline__ int wrap_phi(int phi, int n_phi) {   // phi may be any int; result in [0, n_phi)
+    int r = phi % n_phi;
+    return r < 0 ? r + n_phi : r;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -471,8 +497,12 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
 }
 
 __global__ void __launch_bounds__(kThreads, 1) k_convolve(const ConvParams p) {
+#ifndef ARKCOS_HOST_EMU
     extern __shared__ uint4 smem4[];
     char* smem = reinterpret_cast<char*>(smem4);
+#else
+    char* smem = reinterpret_cast<char*>(emu::g_smem);
+#endif
     const Item it = p.items[blockIdx.x];
     const float* in = p.in + (long long)blockIdx.y * p.map_stride;
     float* out = p.out + (long long)blockIdx.y * p.map_stride;

@@ -1,0 +1,160 @@
+// emu_main.cpp - HOST EMULATION harness of the arkcos CUDA kernels.  Test infrastructure only.
+//
+// Compiles paper_1211_3556_b200/csrc/arkcos_kernels.cuh (the product's kernel source, unchanged) and
+// arkcos_schedule.cpp for the host against tests/emu/stub/cuda_runtime.h and runs, for one plan:
+//   k_generate_weights  ->  k_convolve  (every work item, one CTA at a time, one OS thread per CUDA
+//   thread, real barriers for __syncthreads / __syncwarp, cp.async performed only at its wait).
+// Shared memory is a heap block of exactly the launch's dynamic size (AddressSanitizer sees overruns),
+// every ld.shared wrapper checks bounds and alignment, every cp.async source must lie in a registered
+// global buffer.  Shared memory and the output start as NaN, so a value consumed before it was staged
+// shows up in the result.
+//
+//   emu_arkcos n_theta n_phi theta_cut n_table table.f64 in.f32 out.f32 [only_wide|only_narrow]
+//
+// It does not replace the GPU parity tests: it checks the index logic (windows, staging, wrap-around,
+// pass structure, weight layout), not the compiled SASS.
+#include <barrier>
+#include <memory>
+#include <mutex>
+#include <thread>
+
+#include "cuda_runtime.h"
+
+#include "arkcos_internal.h"
+#include "arkcos_kernels.cuh"
+
+namespace emu {
+thread_local uint3 t_threadIdx, t_blockIdx;
+dim3 g_blockDim, g_gridDim;
+unsigned char* g_smem = nullptr;
+size_t g_smem_bytes = 0;
+
+static std::unique_ptr<std::barrier<>> g_cta_barrier;
+static std::vector<std::unique_ptr<std::barrier<>>> g_warp_barriers;
+struct Range { const unsigned char* lo; const unsigned char* hi; };
+static std::vector<Range> g_global;
+
+[[noreturn]] void fail(const char* what, long a, long b) {
+    std::fprintf(stderr, "EMU FAILURE: %s (%ld, %ld) block %u thread %u\n", what, a, b, t_blockIdx.x, t_threadIdx.x);
+    std::_Exit(3);
+}
+void sync_threads() { g_cta_barrier->arrive_and_wait(); }
+void sync_warp() { g_warp_barriers[t_threadIdx.x >> 5]->arrive_and_wait(); }
+void check_global(const void* p, size_t bytes) {
+    const unsigned char* q = (const unsigned char*)p;
+    if ((uintptr_t)q % 16) fail("misaligned global access of cp.async", (long)((uintptr_t)q % 16), (long)bytes);
+    for (const Range& r : g_global)
+        if (q >= r.lo && q + bytes <= r.hi) return;
+    fail("cp.async source outside every global buffer", 0, (long)bytes);
+}
+
+struct Pending { uint32_t dst; const void* src; };
+static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
+static thread_local std::vector<Pending> t_open;                  // not yet committed
+void cp_async_enqueue(uint32_t dst, const void* src) {
+    (void)smem_at(dst, 16);
+    check_global(src, 16);
+    t_open.push_back(Pending{dst, src});
+}
+void cp_async_commit_group() { t_groups.push_back(std::move(t_open)); t_open.clear(); }
+static void perform(const std::vector<Pending>& g) {
+    for (const Pending& c : g) std::memcpy(smem_at(c.dst, 16), c.src, 16);
+}
+void cp_async_wait(int keep_groups) {
+    if (keep_groups == 0) {            // wait_all / wait_group 0: everything, committed or not
+        for (auto& g : t_groups) perform(g);
+        t_groups.clear();
+        perform(t_open); t_open.clear();
+        return;
+    }
+    while ((int)t_groups.size() > keep_groups) { perform(t_groups.front()); t_groups.erase(t_groups.begin()); }
+}
+static void thread_exit_check() {
+    if (!t_open.empty() || !t_groups.empty()) fail("thread exits with cp.async copies it never waited for", (long)t_groups.size(), 0);
+}
+
+// run one CTA of `threads` threads
+template <typename F>
+static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_bytes, F&& body) {
+    g_smem_bytes = smem_bytes;
+    g_smem = (unsigned char*)std::malloc(smem_bytes ? smem_bytes : 16);
+    std::memset(g_smem, 0xFF, smem_bytes);                        // NaN pattern
+    g_blockDim = dim3(threads);
+    g_cta_barrier = std::make_unique<std::barrier<>>((std::ptrdiff_t)threads);
+    g_warp_barriers.clear();
+    for (unsigned w = 0; w < threads / 32; w++) g_warp_barriers.push_back(std::make_unique<std::barrier<>>(32));
+    std::vector<std::thread> pool;
+    for (unsigned t = 0; t < threads; t++)
+        pool.emplace_back([&, t] {
+            t_threadIdx = uint3{t, 0, 0}; t_blockIdx = uint3{bx, by, 0};
+            body();
+            thread_exit_check();
+        });
+    for (auto& th : pool) th.join();
+    std::free(g_smem);
+    g_smem = nullptr;
+}
+}  // namespace emu
+
+template <typename T>
+static std::vector<T> read_file(const char* path, size_t n) {
+    std::vector<T> v(n);
+    FILE* f = std::fopen(path, "rb");
+    if (!f || std::fread(v.data(), sizeof(T), n, f) != n) { std::fprintf(stderr, "cannot read %s\n", path); std::exit(2); }
+    std::fclose(f);
+    return v;
+}
+
+int main(int argc, char** argv) {
+    using namespace arkcos;
+    if (argc < 8) { std::fprintf(stderr, "usage: emu_arkcos n_theta n_phi theta_cut n_table table.f64 in.f32 out.f32 [only_wide|only_narrow]\n"); return 2; }
+    const int n_theta = std::atoi(argv[1]), n_phi = std::atoi(argv[2]);
+    const double theta_cut = std::atof(argv[3]);
+    const int n_table = std::atoi(argv[4]);
+    const std::string only = argc > 8 ? argv[8] : "";
+    std::vector<double> table = read_file<double>(argv[5], (size_t)n_table);
+    const size_t n_pix = (size_t)n_theta * n_phi;
+    std::vector<float> in = read_file<float>(argv[6], n_pix);
+    std::vector<float> out(n_pix, std::nanf(""));
+
+    Schedule s;
+    const int rc = build_schedule(n_theta, n_phi, theta_cut, 148, s);
+    if (rc != 0) { std::fprintf(stderr, "build_schedule failed: %d\n", rc); return 2; }
+    if (s.smem_bytes > (size_t)kSmemBudget) { std::fprintf(stderr, "shared memory over budget\n"); return 2; }
+    std::vector<float> weights((size_t)s.weight_slots + 4, 0.0f);
+    emu::g_global = {{(const unsigned char*)in.data(), (const unsigned char*)(in.data() + in.size())},
+                     {(const unsigned char*)weights.data(), (const unsigned char*)(weights.data() + weights.size())},
+                     {(const unsigned char*)s.pairs.data(), (const unsigned char*)(s.pairs.data() + s.pairs.size())}};
+
+    // ---- S2: weight generator ----------------------------------------------------------------------
+    GenParams g;
+    g.units = s.gen_units.data(); g.s2 = s.s2.data(); g.table = table.data(); g.weights = weights.data();
+    g.n_units = (int)s.gen_units.size(); g.n_phi = n_phi; g.n_table = n_table;
+    g.t_scale = (double)(n_table - 1) / theta_cut; g.table_in_smem = 1;
+    const int gen_grid = 4;
+    emu::g_gridDim = dim3(gen_grid);
+    for (int b = 0; b < gen_grid; b++)
+        emu::run_cta((unsigned)b, 0, kGenThreads, (size_t)n_table * sizeof(double), [&] { k_generate_weights(g); });
+
+    // ---- S3: convolution, one CTA per work item ------------------------------------------------------
+    ConvParams c;
+    c.in = in.data(); c.out = out.data(); c.pairs = s.pairs.data(); c.items = s.items.data(); c.weights = weights.data();
+    c.ring_w_off = s.ring_w_off.data(); c.ring_slots = s.ring_slots.data();
+    c.n_theta = n_theta; c.n_phi = n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
+    c.map_stride = (long long)n_pix;
+    emu::g_global.push_back({(const unsigned char*)s.ring_w_off.data(), (const unsigned char*)(s.ring_w_off.data() + s.ring_w_off.size())});
+    emu::g_gridDim = dim3((unsigned)s.items.size());
+    int n_wide = 0, n_narrow = 0;
+    for (size_t b = 0; b < s.items.size(); b++) {
+        const bool wide = s.items[b].kind == kWide;
+        if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
+        (wide ? n_wide : n_narrow)++;
+        emu::run_cta((unsigned)b, 0, kThreads, s.smem_bytes, [&] { k_convolve(c); });
+    }
+    FILE* f = std::fopen(argv[7], "wb");
+    if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
+    std::fclose(f);
+    std::printf("emu ok: R %d first_narrow %d n_north %d narrow_f_log2 %d items wide %d narrow %d smem %zu weight_slots %llu\n", s.R,
+                s.first_narrow, s.n_north, s.narrow_f_log2, n_wide, n_narrow, s.smem_bytes, (unsigned long long)s.weight_slots);
+    return 0;
+}

@@ -1,0 +1,59 @@
+// Stub <cuda_runtime.h> for the HOST EMULATION of the arkcos CUDA kernels (tests/emu/).  Test
+// infrastructure only: it lets `-m "not gpu"` tests execute the very kernel source of
+// paper_1211_3556_b200/csrc/arkcos_kernels.cuh on CPU threads (one OS thread per CUDA thread, one CTA
+// at a time) with bounds- and alignment-checked shared memory, so that index logic can be checked
+// against the oracle on machines without a GPU.  Nothing in the product links or includes this.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#define __global__
+#define __device__
+#define __host__
+#define __forceinline__ inline __attribute__((always_inline))
+#define __launch_bounds__(...)
+#define __shared__
+#define __restrict__
+
+struct dim3 { unsigned x = 1, y = 1, z = 1; dim3(unsigned a = 1, unsigned b = 1, unsigned c = 1) : x(a), y(b), z(c) {} };
+struct uint3 { unsigned x, y, z; };
+struct alignas(16) float4 { float x, y, z, w; };
+struct alignas(16) uint4 { unsigned x, y, z, w; };
+static inline float4 make_float4(float a, float b, float c, float d) { return float4{a, b, c, d}; }
+
+using std::max;
+using std::min;
+
+namespace emu {
+extern thread_local uint3 t_threadIdx, t_blockIdx;
+extern dim3 g_blockDim, g_gridDim;
+extern unsigned char* g_smem;         // base of the CTA's dynamic shared memory
+extern size_t g_smem_bytes;           // its size for the current launch
+void sync_threads();                  // CTA barrier
+void sync_warp();                     // warp barrier
+[[noreturn]] void fail(const char* what, long a, long b);
+// checked shared-memory window [addr, addr + bytes), aligned to `bytes`
+static inline unsigned char* smem_at(uint32_t addr, uint32_t bytes) {
+    if ((size_t)addr + bytes > g_smem_bytes) fail("shared-memory access out of bounds", addr, bytes);
+    if (addr % bytes) fail("misaligned shared-memory access", addr, bytes);
+    return g_smem + addr;
+}
+void check_global(const void* p, size_t bytes);   // must lie inside a registered global buffer, 16-byte aligned
+// cp.async emulation: copies are queued per thread and only performed by the wait calls
+void cp_async_enqueue(uint32_t dst, const void* src);
+void cp_async_commit_group();
+void cp_async_wait(int keep_groups);
+}  // namespace emu
+
+#define threadIdx (emu::t_threadIdx)
+#define blockIdx (emu::t_blockIdx)
+#define blockDim (emu::g_blockDim)
+#define gridDim (emu::g_gridDim)
+static inline void __syncthreads() { emu::sync_threads(); }
+static inline void __syncwarp() { emu::sync_warp(); }
+static inline size_t __cvta_generic_to_shared(const void* p) { return (size_t)((const unsigned char*)p - emu::g_smem); }
