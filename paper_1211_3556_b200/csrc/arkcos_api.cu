@@ -40,7 +40,7 @@ struct arkcos_plan {
     Item* d_items = nullptr;
     GenUnit* d_units = nullptr;
     double *d_s2 = nullptr, *d_table = nullptr;
-    uint32_t *d_ring_w_off = nullptr, *d_ring_slots = nullptr;
+    NarrowRun* d_runs = nullptr;
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging, lazily allocated
     size_t device_bytes = 0;
@@ -77,7 +77,7 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
 arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
-    c.ring_w_off = pl->d_ring_w_off; c.ring_slots = pl->d_ring_slots;
+    c.runs = pl->d_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
     c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
     c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
     if (pl->sched.items.empty()) return ARKCOS_OK;
@@ -123,8 +123,7 @@ const char* arkcos_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!pl) return ARKCOS_OK;
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
-        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_ring_w_off);
-        cudaFree(pl->d_ring_slots); cudaFree(pl->d_s2); cudaFree(pl->d_table);
+        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
         for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
         (void)cudaGetLastError();
@@ -174,8 +173,7 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
         if ((st = upload(pl, &pl->d_pairs, s.pairs)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_items, s.items)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_units, s.gen_units)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_ring_w_off, s.ring_w_off)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_ring_slots, s.ring_slots)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_runs, s.runs)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_s2, s.s2)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_table, pl->table)) != ARKCOS_OK) break;
         {

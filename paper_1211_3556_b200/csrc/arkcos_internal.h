@@ -55,6 +55,15 @@ struct PairDesc {
     int32_t half;     // D (taps -D..D inside theta_cut); n_phi = whole ring; -1 = empty
 };
 
+// Kernel-ready form of a NARROW ring pair (what conv_narrow stages instead of PairDesc): the run enters
+// the unrolled step chain at step k0 = (32 + start) / 2 and executes n = ntaps / 2 steps.
+struct NarrowRun {
+    int32_t wq_rel;   // byte offset of the run's weights in the ring's weight block, minus 8 * k0
+    int32_t k0;       // entry step
+    int32_t n;        // steps; 0 = nothing to do
+    int32_t pad_;
+};
+
 enum ItemKind : int16_t { kWide = 0, kNarrow = 1 };
 
 // One CTA of the convolution launch.
@@ -66,6 +75,7 @@ struct Item {
     int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings, S rings per pass
     int32_t nrings;   // kNarrow: rings of the band; negative = the band is the southern mirror of
                       //   northern rings [i0, i0 - nrings)
+    int32_t wcopy;    // kNarrow: floats of a ring's weight block to stage (max over the band; multiple of 4)
 };
 
 // Work unit of the weight generator (one warp) for one ring pair: `count` taps d0, d0+1, ...
@@ -92,6 +102,8 @@ struct Schedule {
     std::vector<double> a_r;                // [R+1] sin^2(r dtheta / 2)
     std::vector<double> s2;                 // [n_phi/2+1] sin^2(d dphi / 2)
     std::vector<PairDesc> pairs;            // [n_north][2R+1]
+    std::vector<NarrowRun> runs;            // [n_north - first_narrow][2R+1]
+    uint32_t narrow_w_base = 0;             // weights of narrow ring i start at narrow_w_base + (i - first_narrow) * narrow_wslot
     std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
     std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows, padded to 4)
     std::vector<Item> items;                // cost-sorted, heaviest first

@@ -88,9 +88,10 @@ struct ConvParams {
     const PairDesc* pairs;
     const Item* items;
     const float* weights;
-    const uint32_t* ring_w_off;
-    const uint32_t* ring_slots;
+    const NarrowRun* runs;   // [n_north - first_narrow][2R+1]
     int n_theta, n_phi, R;
+    int first_narrow;        // first northern ring of the narrow class
+    uint32_t narrow_w_base;  // its weights start here; one block of wslot floats per narrow ring
     int wslot;               // floats per ring in the narrow weight buffers
     long long map_stride;    // elements between consecutive maps of a batch
 };
@@ -120,6 +121,9 @@ template <int OFF>
 __device__ __forceinline__ void lds64i(float& a, float& b, const uint32_t addr) {
     asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(a), "=f"(b) : "r"(addr), "n"(OFF));
 }
+__device__ __forceinline__ void lds128u(int& a, int& b, int& c, int& d, const uint32_t addr) {
+    asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr));
+}
 #else
 __device__ __forceinline__ void cp_async16(const uint32_t smem_dst, const void* gmem_src) { emu::cp_async_enqueue(smem_dst, gmem_src); }
 __device__ __forceinline__ void cp_async_commit() { emu::cp_async_commit_group(); }
@@ -136,6 +140,10 @@ template <int OFF>
 __device__ __forceinline__ void lds64i(float& a, float& b, const uint32_t addr) {
     const float* q = reinterpret_cast<const float*>(emu::smem_at(addr + (uint32_t)OFF, 8));
     a = q[0]; b = q[1];
+}
+__device__ __forceinline__ void lds128u(int& a, int& b, int& c, int& d, const uint32_t addr) {
+    const int* q = reinterpret_cast<const int*>(emu::smem_at(addr, 16));
+    a = q[0]; b = q[1]; c = q[2]; d = q[3];
 }
 #endif
 
@@ -415,7 +423,7 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     const int slot_bytes = narrow_slot_bytes(it.f_log2);
     const uint32_t rows = (uint32_t)__cvta_generic_to_shared(smem);
     float* wbuf = reinterpret_cast<float*>(smem + (size_t)NS * slot_bytes);               // [2][S][wslot]
-    PairDesc* pdbuf = reinterpret_cast<PairDesc*>(wbuf + 2 * (size_t)S * p.wslot);        // [2][S][W]
+    NarrowRun* pdbuf = reinterpret_cast<NarrowRun*>(wbuf + 2 * (size_t)S * p.wslot);      // [2][S][W]
     const uint32_t wbuf_addr = (uint32_t)__cvta_generic_to_shared(wbuf);
     const uint32_t pdbuf_addr = (uint32_t)__cvta_generic_to_shared(pdbuf);
     const int lam0 = it.i0, lam_end = it.i0 + nr;
@@ -439,17 +447,18 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
             if (phi >= p.n_phi) phi -= p.n_phi;
         }
     };
-    // weights and pair descriptors of the S rings of a pass -> buffer b
+    // weights and run descriptors of the S rings of a pass -> buffer b (no dependent global loads:
+    // both live at computable addresses)
+    const int n4 = it.wcopy >> 2;
     auto stage_ring_tables = [&](const int pass, const int b) {
         for (int rs = 0; rs < S; rs++) {
             const int lam = lam0 + pass * S + rs;
             if (lam >= lam_end) break;
-            const PairDesc* psrc = p.pairs + (size_t)lam * W;
-            const uint32_t pdst = pdbuf_addr + (uint32_t)(((b * S + rs) * W) * sizeof(PairDesc));
+            const NarrowRun* psrc = p.runs + (size_t)(lam - p.first_narrow) * W;
+            const uint32_t pdst = pdbuf_addr + (uint32_t)(((b * S + rs) * W) * sizeof(NarrowRun));
             for (int q = threadIdx.x; q < W; q += kThreads) cp_async16(pdst + 16 * q, psrc + q);
-            const float* src = p.weights + p.ring_w_off[lam];
+            const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
             const uint32_t dst = wbuf_addr + (uint32_t)(((b * S + rs) * p.wslot) * 4);
-            const int n4 = (int)(p.ring_slots[lam] >> 2);
             for (int q = threadIdx.x; q < n4; q += kThreads) cp_async16(dst + 16 * q, src + 4 * q);
         }
     };
@@ -472,18 +481,23 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
             for (int m = 0; m < kLaneP; m++) { a0[m] = 0.f; a1[m] = 0.f; }
             const int tb = (pass & 1) * S + s;
             const uint32_t wring = wbuf_addr + (uint32_t)(tb * p.wslot * 4);
-            const PairDesc* spd = pdbuf + (size_t)tb * W;
-            uint32_t w0 = 0xFFFFFFFFu;
+            const uint32_t spd = pdbuf_addr + (uint32_t)(tb * W * sizeof(NarrowRun));
             int slot = (lam - p.R) % NS; if (slot < 0) slot += NS;
+            uint32_t zt = rows + (uint32_t)(slot * slot_bytes) + lane_tile;
+            const uint32_t zt_end = rows + (uint32_t)(NS * slot_bytes) + lane_tile;
+            // Run descriptors are double buffered in registers: the descriptor of run r+1 is loaded into
+            // the other set while run r executes, and only copied out of it one run later.
+            int dA[4], dB[4];
+            lds128u(dA[0], dA[1], dA[2], dA[3], spd);
+#pragma unroll 1
             for (int r = 0; r < W; r++) {
-                const PairDesc pd = spd[r];
-                if (pd.ntaps != 0) {
-                    if (w0 == 0xFFFFFFFFu) w0 = pd.w_off;      // first stored row = start of the ring's weights
-                    const int k0 = (kHaloNarrow + pd.start) >> 1;
-                    narrow_row(a0, a1, rows + (uint32_t)(slot * slot_bytes) + lane_tile,
-                               wring + 4u * (pd.w_off - w0) - 8u * (uint32_t)k0, k0, pd.ntaps >> 1);
-                }
-                if (++slot == NS) slot = 0;
+                const uint32_t nxt = spd + (uint32_t)((r + 1 < W ? r + 1 : r) * sizeof(NarrowRun));
+                int wq_rel, k0, n;
+                if (r & 1) { wq_rel = dB[0]; k0 = dB[1]; n = dB[2]; lds128u(dA[0], dA[1], dA[2], dA[3], nxt); }
+                else { wq_rel = dA[0]; k0 = dA[1]; n = dA[2]; lds128u(dB[0], dB[1], dB[2], dB[3], nxt); }
+                if (n != 0) narrow_row(a0, a1, zt, wring + (uint32_t)wq_rel, k0, n);
+                zt += (uint32_t)slot_bytes;
+                if (zt == zt_end) zt -= (uint32_t)(NS * slot_bytes);
             }
             const int phi = it.k0 + f * kWarpSpan + lane * kLaneP;
             float* orow = out + (size_t)(south ? p.n_theta - 1 - lam : lam) * p.n_phi + phi;

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 
 #include "arkcos_internal.h"
 
@@ -134,18 +135,23 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     }
     int nf_cap = 0;                                           // largest useful F of the narrow tiles
     while (nf_cap < 3 && (kWarpSpan << nf_cap) < n_phi) nf_cap++;
+    if (const char* e = std::getenv("ARKCOS_NARROW_F_LOG2")) nf_cap = std::min(nf_cap, std::max(0, std::atoi(e)));   // tuning knob
     s.narrow_f_log2 = -1;
     for (int fl = nf_cap; fl >= 0; fl--)
         if (narrow_smem_bytes(fl, s.R, s.narrow_wslot) <= (size_t)kSmemBudget) { s.narrow_f_log2 = fl; break; }
     if (s.narrow_f_log2 < 0 || s.n_north - s.first_narrow < 1) { s.first_narrow = s.n_north; s.narrow_f_log2 = 0; }
 
     // ---- weight layout ------------------------------------------------------------------------------
+    // WIDE rings: one contiguous block per ring.  NARROW rings: blocks at a uniform stride of narrow_wslot
+    // floats, so that conv_narrow can stage a ring's block without reading an offset table first.
     unsigned long long w_off = 0;
     std::vector<unsigned long long> ring_slots(s.n_north, 0);  // stored taps per output phi
     s.ring_w_off.assign(s.n_north, 0u); s.ring_slots.assign(s.n_north, 0u);
     for (int i = 0; i < s.n_north; i++) {
         const bool wide = i < s.first_narrow;
-        bool first = true;
+        if (i == s.first_narrow) s.narrow_w_base = (uint32_t)w_off;
+        const unsigned long long ring_base = w_off;
+        s.ring_w_off[i] = (uint32_t)w_off;
         for (int r = 0; r < W; r++) {
             PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half < 0) continue;
@@ -153,14 +159,25 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             const unsigned long long floats = (unsigned long long)p.ntaps;
             if (w_off + floats > 0xFFFFFFF0ull) return 4;
             p.w_off = (uint32_t)w_off;
-            if (first) { s.ring_w_off[i] = p.w_off; first = false; }   // ring-contiguous weight block
             w_off += floats;
             ring_slots[i] += (unsigned long long)p.ntaps;
         }
-        w_off = (w_off + 3) & ~3ull;                                   // every ring's block is 16-byte aligned
         s.ring_slots[i] = (uint32_t)((ring_slots[i] + 3) & ~3ull);
+        if (wide) w_off = (w_off + 3) & ~3ull;                         // every ring's block is 16-byte aligned
+        else w_off = ring_base + (unsigned long long)s.narrow_wslot;
+        if (w_off > 0xFFFFFFF0ull) return 4;
     }
     s.weight_slots = w_off;
+    s.runs.assign((size_t)(s.n_north - s.first_narrow) * W, NarrowRun{0, 0, 0, 0});
+    for (int i = s.first_narrow; i < s.n_north; i++)
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (p.ntaps == 0) continue;
+            NarrowRun& u = s.runs[(size_t)(i - s.first_narrow) * W + r];
+            u.k0 = (kHaloNarrow + p.start) / 2;
+            u.n = p.ntaps / 2;
+            u.wq_rel = 4 * (int32_t)(p.w_off - s.ring_w_off[i]) - 8 * u.k0;
+        }
 
     // ---- generator work units: one warp writes up to kGenUnitTaps taps (steps) of one ring pair -----
     for (int i = 0; i < s.n_north; i++) {
@@ -200,7 +217,7 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
                 const int valid = std::min(L, n_phi - k0);
                 const double cost = (double)ring_slots[i] * (double)valid + 4000.0;
                 for (int hemi = 0; hemi < (i_s != i ? 2 : 1); hemi++) {
-                    tmp.push_back(Tmp{Item{hemi ? i_s : i, k0, (int16_t)fl, (int16_t)kWide, 1}, cost});
+                    tmp.push_back(Tmp{Item{hemi ? i_s : i, k0, (int16_t)fl, (int16_t)kWide, 1, 0}, cost});
                     s.fma_slots += ring_slots[i] * (unsigned long long)L;
                     s.fma_slots_wide += ring_slots[i] * (unsigned long long)L;
                 }
@@ -224,9 +241,10 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
                 const int nb = hemi ? b_south : b;
                 if (nb <= 0) continue;
                 c = 0.0;
-                for (int q = 0; q < nb; q++) c += (double)ring_slots[i + q] * (double)L;
+                uint32_t wcopy = 4;
+                for (int q = 0; q < nb; q++) { c += (double)ring_slots[i + q] * (double)L; wcopy = std::max(wcopy, s.ring_slots[i + q]); }
                 for (int k0 = 0; k0 < n_phi; k0 += L) {
-                    tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, hemi ? -nb : nb}, c + 4000.0});
+                    tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, hemi ? -nb : nb, (int32_t)wcopy}, c + 4000.0});
                     for (int q = 0; q < nb; q++) s.fma_slots += ring_slots[i + q] * (unsigned long long)L;
                 }
             }

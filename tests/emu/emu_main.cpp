@@ -139,10 +139,10 @@ int main(int argc, char** argv) {
     // ---- S3: convolution, one CTA per work item ------------------------------------------------------
     ConvParams c;
     c.in = in.data(); c.out = out.data(); c.pairs = s.pairs.data(); c.items = s.items.data(); c.weights = weights.data();
-    c.ring_w_off = s.ring_w_off.data(); c.ring_slots = s.ring_slots.data();
+    c.runs = s.runs.data(); c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
     c.n_theta = n_theta; c.n_phi = n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
     c.map_stride = (long long)n_pix;
-    emu::g_global.push_back({(const unsigned char*)s.ring_w_off.data(), (const unsigned char*)(s.ring_w_off.data() + s.ring_w_off.size())});
+    emu::g_global.push_back({(const unsigned char*)s.runs.data(), (const unsigned char*)(s.runs.data() + s.runs.size())});
     emu::g_gridDim = dim3((unsigned)s.items.size());
     int n_wide = 0, n_narrow = 0;
     for (size_t b = 0; b < s.items.size(); b++) {

@@ -1,0 +1,92 @@
+"""Host emulation of the CUDA kernels against the FP64 oracle (no GPU needed).
+
+tests/emu/ compiles the product's kernel source (csrc/arkcos_kernels.cuh + arkcos_schedule.cpp) for the
+host - one OS thread per CUDA thread, checked shared memory, cp.async performed at its wait - and runs
+generator + convolution for a whole plan.  This checks the INDEX LOGIC of the kernels (windows, lane-tile
+layout, wrap-around, band marching, tap splits, weight layout) with the north_star tolerance; the compiled
+SASS is checked by the `gpu` parity tests.  The emulator evaluates the same FP32 fmaf in the same order as
+the kernel, so the error it shows is the kernel's accumulation error.
+"""
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from oracle import oracle
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+EMU_DIR = os.path.join(ROOT, "tests", "emu")
+CSRC = os.path.join(ROOT, "paper_1211_3556_b200", "csrc")
+EMU_BIN = os.path.join(EMU_DIR, "emu_arkcos")
+
+
+@pytest.fixture(scope="module")
+def emu_bin():
+    srcs = [os.path.join(EMU_DIR, "emu_main.cpp"), os.path.join(CSRC, "arkcos_schedule.cpp")]
+    deps = srcs + [os.path.join(CSRC, "arkcos_kernels.cuh"), os.path.join(CSRC, "arkcos_internal.h"),
+                   os.path.join(EMU_DIR, "stub", "cuda_runtime.h")]
+    if not os.path.exists(EMU_BIN) or any(os.path.getmtime(d) > os.path.getmtime(EMU_BIN) for d in deps):
+        cmd = ["g++", "-std=c++20", "-O1", "-g", "-fsanitize=address", "-fno-omit-frame-pointer", "-pthread",
+               "-DARKCOS_HOST_EMU", "-Wno-unknown-pragmas", "-I", os.path.join(EMU_DIR, "stub"), "-I", CSRC] + srcs + ["-o", EMU_BIN]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        assert res.returncode == 0, res.stderr[-3000:]
+    return EMU_BIN
+
+
+def emulate(emu, tmp_path, x32, table, theta_cut, only=None):
+    n_theta, n_phi = x32.shape
+    t, i, o = (str(tmp_path / n) for n in ("table.f64", "in.f32", "out.f32"))
+    np.ascontiguousarray(table, dtype=np.float64).tofile(t)
+    np.ascontiguousarray(x32, dtype=np.float32).tofile(i)
+    cmd = [emu, str(n_theta), str(n_phi), repr(float(theta_cut)), str(table.size), t, i, o] + ([only] if only else [])
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0, (res.stdout + res.stderr)[-3000:]
+    return np.fromfile(o, dtype=np.float32).reshape(n_theta, n_phi).astype(np.float64), res.stdout
+
+
+def gaussian_table(sigma, theta_cut, n):
+    th = np.linspace(0.0, theta_cut, n)
+    return np.exp(-0.5 * (th / sigma) ** 2) / (2.0 * math.pi * sigma * sigma)
+
+
+# (n_theta, n_phi, sigma [deg], cut [sigma]): chosen so that theta_cut / dtheta is not an integer (DESIGN R3)
+CASES = [
+    (64, 128, 3.0, 3.0),      # configs[0]: wide polar rings + one narrow band per hemisphere, ragged warp tile
+    (65, 128, 3.0, 3.0),      # odd n_theta: the equator ring is its own mirror
+    (200, 512, 1.27, 3.0),    # R = 4, several narrow passes
+    (96, 1024, 1.43, 2.5),    # R = 1, whole warp tile
+    (301, 256, 0.9, 4.1),     # R = 6, odd n_theta, narrow windows up to the +-32 limit
+]
+
+
+@pytest.mark.parametrize("n_theta,n_phi,sigma_deg,cut_sigmas", CASES)
+def test_emulated_kernels_match_oracle(emu_bin, tmp_path, n_theta, n_phi, sigma_deg, cut_sigmas):
+    sigma = math.radians(sigma_deg)
+    cut = cut_sigmas * sigma
+    assert abs(cut / (math.pi / n_theta) - round(cut / (math.pi / n_theta))) > 1e-3
+    table = gaussian_table(sigma, cut, 1024)
+    x32 = np.random.default_rng(1000 + n_theta).standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    assert not np.isnan(got).any(), "an output was never written or consumed unstaged shared memory\n" + log
+    expect = oracle.convolve(x32, table, cut, level=1)
+    rms = math.sqrt((expect ** 2).mean())
+    rel = math.sqrt(((got - expect) ** 2).mean()) / rms
+    mx = float(np.abs(got - expect).max()) / rms
+    assert rel <= 1e-6 and mx <= 1e-5, (rel, mx, log)
+
+
+def test_emulated_two_phi_tiles_and_oscillating_kernel(emu_bin, tmp_path):
+    """n_phi = 2048: two warp tiles per ring (F = 2 narrow sub-tiles, wrap-around across the tile seam), with a
+    sign-changing kernel so that a misplaced tap cannot hide behind a smooth weight profile."""
+    n_theta, n_phi = 80, 2048
+    cut = math.radians(4.3)
+    th = np.linspace(0.0, cut, 2048)
+    table = np.cos(7.0 * th / cut) * np.exp(-0.5 * (th / (0.4 * cut)) ** 2) * 50.0
+    x32 = np.random.default_rng(7).standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    expect = oracle.convolve(x32, table, cut, level=1)
+    rms = math.sqrt((expect ** 2).mean())
+    assert not np.isnan(got).any(), log
+    assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
