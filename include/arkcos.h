@@ -76,6 +76,24 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan **plan, int n_theta, int n_phi, 
                                     int n_table, double theta_cut_rad, unsigned flags);
 
 /*
+ * arkcos_plan_create_biased - as arkcos_plan_create_ex, for the paper's two-zone interpolation table
+ * (§3: "we place half the available interpolation nodes within the first 1/16th of the
+ * available support", because the split kernel oscillates fastest at small angles).
+ *   k_table          HOST, n_table samples at the nodes
+ *                       theta_m = m * theta_split / m_split                                  (m <= m_split)
+ *                       theta_m = theta_split + (m - m_split) * (theta_cut - theta_split) / (n_table - 1 - m_split)
+ *                    i.e. node m_split sits exactly at theta_split and the nodes are uniform on either side;
+ *                    K is the linear interpolant between neighbouring nodes, as for the uniform table
+ *   m_split          1 <= m_split <= n_table - 2   (the paper: m_split = (n_table - 1) / 2)
+ *   theta_split_rad  0 < theta_split < theta_cut   (the paper: theta_cut / 16)
+ * Everything else (support, ring areas, schedule, kernels) is unchanged: only step S2's table lookup differs.
+ * Errors: as arkcos_plan_create_ex, plus EINVAL for an m_split / theta_split outside the ranges above.
+ */
+arkcos_status arkcos_plan_create_biased(arkcos_plan **plan, int n_theta, int n_phi, const double *k_table,
+                                        int n_table, double theta_cut_rad, int m_split, double theta_split_rad,
+                                        unsigned flags);
+
+/*
  * arkcos_convolve - the hot path, steps S2 (weight generator) + S3/S3w (convolution kernels).
  *   d_in   DEVICE, [n_theta][n_phi] FP32, 16-byte aligned, read only
  *   d_out  DEVICE, same shape, 16-byte aligned, fully overwritten; must not overlap d_in

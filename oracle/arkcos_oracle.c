@@ -31,6 +31,14 @@
  *      ring, a phi window padded by 2 pixels each side (or the whole ring), still applying step 3 to
  *      every visited pair and reusing no weight between output pixels.
  *
+ * Two-zone ("biased") table, PAPER.md:L88 (§3): "we place half the available interpolation nodes within
+ * the first 1/16th of the available support".  oracle_convolve_biased takes the node index m_split that
+ * sits exactly at theta_split: nodes 0..m_split are uniform on [0, theta_split], nodes m_split..n-1 are
+ * uniform on [theta_split, theta_cut]; K stays the linear interpolant between neighbouring nodes.  Step 4
+ * then reads  t = gamma/theta_split*m_split  (gamma < theta_split)  or
+ * t = m_split + (gamma-theta_split)/(theta_cut-theta_split)*(n-1-m_split).  m_split = 0 is the uniform
+ * table.  Pinned by tests/test_biased_table.py against numpy.interp over the explicit node positions.
+ *
  * Parity pins (tests/test_oracle_*.py, `-m "not gpu"`): delta-input point values against an
  * independent atan2 angle formula, total area = 4 pi, phi-shift and N/S-mirror equivariance,
  * area-weighted self-adjointness, constant-map and Y_lm closed forms (b_l of the piecewise-linear
@@ -51,6 +59,8 @@
 typedef struct {
     int n_theta, n_phi, n_table;
     double theta_cut, dtheta, dphi;
+    int m_split;             /* 0: uniform table */
+    double theta_split;
     double *sin_t, *cos_t;   /* per ring  */
     double *cos_p, *sin_p;   /* per phi   */
     double *area;            /* per ring  */
@@ -95,7 +105,10 @@ static inline int pair_kernel(const grid_t *g, int i, int k, int j, int kk, doub
     double cochord = sqrt(sx * sx + sy * sy + sz * sz);    /* |n_p + n_q| = 2 cos(gamma/2) */
     double gamma = 2.0 * atan2(chord, cochord);
     if (!(gamma <= g->theta_cut)) return 0;                /* support, inclusive */
-    double t = gamma / g->theta_cut * (double)(g->n_table - 1);
+    double t;
+    if (g->m_split <= 0) t = gamma / g->theta_cut * (double)(g->n_table - 1);
+    else if (gamma < g->theta_split) t = gamma / g->theta_split * (double)g->m_split;
+    else t = (double)g->m_split + (gamma - g->theta_split) / (g->theta_cut - g->theta_split) * (double)(g->n_table - 1 - g->m_split);
     int m = (int)floor(t); if (m > g->n_table - 2) m = g->n_table - 2; if (m < 0) m = 0;
     double f = t - (double)m;
     *kval = (1.0 - f) * g->table[m] + f * g->table[m + 1];
@@ -163,13 +176,17 @@ static long double pixel_level1(const grid_t *g, const double *in, int i, int k,
  *   n_threads  <= 0: OpenMP default
  * Returns ORACLE_OK / ORACLE_EINVAL / ORACLE_ENOMEM.
  */
-int oracle_convolve(int level, int n_theta, int n_phi, const double *table, int n_table, double theta_cut,
-                    const double *in, const long long *pix, long long n_pix, double *out,
-                    unsigned long long *n_pairs, int n_threads) {
+int oracle_convolve_biased(int level, int n_theta, int n_phi, const double *table, int n_table, double theta_cut,
+                           int m_split, double theta_split,
+                           const double *in, const long long *pix, long long n_pix, double *out,
+                           unsigned long long *n_pairs, int n_threads) {
     grid_t g;
     if (!in || !out || (level != 0 && level != 1) || n_pix < 0) return ORACLE_EINVAL;
+    if (m_split < 0 || (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))))
+        return ORACLE_EINVAL;
     int rc = grid_init(&g, n_theta, n_phi, table, n_table, theta_cut);
     if (rc != ORACLE_OK) return rc;
+    g.m_split = m_split; g.theta_split = theta_split;
     long long total = (long long)n_theta * n_phi;
     if (!pix) n_pix = total;
     unsigned long long pairs = 0;
@@ -190,6 +207,13 @@ int oracle_convolve(int level, int n_theta, int n_phi, const double *table, int 
     if (n_pairs) *n_pairs = pairs;
     grid_free(&g);
     return bad ? ORACLE_EINVAL : ORACLE_OK;
+}
+
+/* uniform table: the two-zone entry point with no inner zone */
+int oracle_convolve(int level, int n_theta, int n_phi, const double *table, int n_table, double theta_cut,
+                    const double *in, const long long *pix, long long n_pix, double *out,
+                    unsigned long long *n_pairs, int n_threads) {
+    return oracle_convolve_biased(level, n_theta, n_phi, table, n_table, theta_cut, 0, 0.0, in, pix, n_pix, out, n_pairs, n_threads);
 }
 
 /* exact ring pixel areas A_j, for the area pin (sum_j N_phi A_j = 4 pi) and the adjointness pin */

@@ -43,6 +43,12 @@ def _load():
             ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_double,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
             ctypes.POINTER(ctypes.c_ulonglong), ctypes.c_int]
+        lib.oracle_convolve_biased.restype = ctypes.c_int
+        lib.oracle_convolve_biased.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_double,
+            ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
+            ctypes.POINTER(ctypes.c_ulonglong), ctypes.c_int]
         lib.oracle_ring_area.restype = ctypes.c_int
         lib.oracle_ring_area.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
         lib.oracle_max_threads.restype = ctypes.c_int
@@ -64,8 +70,11 @@ def ring_area(n_theta: int, n_phi: int) -> np.ndarray:
 
 def convolve(map_in: np.ndarray, table: np.ndarray, theta_cut: float, *, level: int = 1,
              pixels: Optional[np.ndarray] = None, n_threads: int = 0,
-             return_pairs: bool = False):
+             return_pairs: bool = False, m_split: int = 0, theta_split: float = 0.0):
     """out = map (*) K(theta <= theta_cut), FP64.
+
+    m_split > 0: two-zone table: node m_split sits at theta_split, nodes are uniform on
+    either side of it.
 
     map_in  [n_theta][n_phi], any float dtype (promoted exactly to FP64)
     table   K at theta_m = m*theta_cut/(n_table-1), FP64
@@ -84,9 +93,10 @@ def convolve(map_in: np.ndarray, table: np.ndarray, theta_cut: float, *, level: 
         pix_ptr, n_pix = pix.ctypes.data, pix.size
         out = np.empty(pix.shape, dtype=np.float64)
     pairs = ctypes.c_ulonglong(0)
-    rc = _load().oracle_convolve(level, n_theta, n_phi, t.ctypes.data, t.size, float(theta_cut),
-                                 x.ctypes.data, pix_ptr, n_pix, out.ctypes.data,
-                                 ctypes.byref(pairs), int(n_threads))
+    rc = _load().oracle_convolve_biased(level, n_theta, n_phi, t.ctypes.data, t.size, float(theta_cut),
+                                        int(m_split), float(theta_split),
+                                        x.ctypes.data, pix_ptr, n_pix, out.ctypes.data,
+                                        ctypes.byref(pairs), int(n_threads))
     if rc != 0:
         raise ValueError(f"oracle_convolve rc={rc}")
     if return_pairs:

@@ -49,6 +49,8 @@ SYMBOLS = [
                                           ctypes.c_int, ctypes.c_double]),
     ("arkcos_plan_create_ex", ctypes.c_int, [ctypes.POINTER(_c_plan_p), ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                              ctypes.c_int, ctypes.c_double, ctypes.c_uint]),
+    ("arkcos_plan_create_biased", ctypes.c_int, [ctypes.POINTER(_c_plan_p), ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                                 ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_double, ctypes.c_uint]),
     ("arkcos_convolve", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     ("arkcos_convolve_batch", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     ("arkcos_convolve_host", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
@@ -103,11 +105,18 @@ def _ptr(t) -> int:
 class Plan:
     """arkcos_plan_create / arkcos_plan_destroy with the same argument meaning as the C ABI."""
 
-    def __init__(self, n_theta: int, n_phi: int, k_table, theta_cut: float, flags: int = PLAN_DEFAULT):
+    def __init__(self, n_theta: int, n_phi: int, k_table, theta_cut: float, flags: int = PLAN_DEFAULT,
+                 m_split: int = 0, theta_split: float = 0.0):
+        """m_split > 0: arkcos_plan_create_biased (two-zone table, node m_split at theta_split)."""
         table = np.ascontiguousarray(k_table, dtype=np.float64)
         self._h = _c_plan_p()
-        _check(lib().arkcos_plan_create_ex(ctypes.byref(self._h), int(n_theta), int(n_phi), table.ctypes.data,
-                                           int(table.size), float(theta_cut), int(flags)), "arkcos_plan_create")
+        if m_split:
+            _check(lib().arkcos_plan_create_biased(ctypes.byref(self._h), int(n_theta), int(n_phi), table.ctypes.data,
+                                                   int(table.size), float(theta_cut), int(m_split), float(theta_split),
+                                                   int(flags)), "arkcos_plan_create_biased")
+        else:
+            _check(lib().arkcos_plan_create_ex(ctypes.byref(self._h), int(n_theta), int(n_phi), table.ctypes.data,
+                                               int(table.size), float(theta_cut), int(flags)), "arkcos_plan_create")
         self.n_theta, self.n_phi = int(n_theta), int(n_phi)
 
     # -- hot path -----------------------------------------------------------------------------

@@ -32,6 +32,8 @@ struct arkcos_plan {
     Schedule sched;
     std::vector<double> table;
     int n_table = 0;
+    int m_split = 0;                  // two-zone table (arkcos_plan_create_biased); 0 = uniform
+    double theta_split = 0.0;
     unsigned flags = 0;
     int device = -1, sm_count = 0;
     bool weights_ready = false;       // cached plans: generator already ran
@@ -68,6 +70,11 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
     g.units = pl->d_units; g.s2 = pl->d_s2; g.table = pl->d_table; g.weights = pl->d_weights;
     g.n_units = (int)pl->sched.gen_units.size(); g.n_phi = pl->sched.n_phi; g.n_table = pl->n_table;
     g.t_scale = (double)(pl->n_table - 1) / pl->sched.theta_cut;
+    g.m_split = pl->m_split; g.theta_split = pl->theta_split; g.t_scale2 = 0.0;
+    if (pl->m_split > 0) {
+        g.t_scale = (double)pl->m_split / pl->theta_split;
+        g.t_scale2 = (double)(pl->n_table - 1 - pl->m_split) / (pl->sched.theta_cut - pl->theta_split);
+    }
     g.table_in_smem = pl->table_in_smem;
     k_generate_weights<<<pl->gen_grid, kGenThreads, pl->gen_smem, st>>>(g);
     CU(cudaGetLastError());
@@ -134,8 +141,15 @@ arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
 
 arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, const double* k_table, int n_table,
                                     double theta_cut, unsigned flags) {
+    return arkcos_plan_create_biased(plan, n_theta, n_phi, k_table, n_table, theta_cut, 0, 0.0, flags);
+}
+
+arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_phi, const double* k_table, int n_table,
+                                        double theta_cut, int m_split, double theta_split, unsigned flags) {
     if (!plan) return ARKCOS_EINVAL;
     *plan = nullptr;
+    if (m_split < 0) return ARKCOS_EINVAL;
+    if (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))) return ARKCOS_EINVAL;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
     if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
@@ -144,6 +158,7 @@ arkcos_status arkcos_plan_create_ex(arkcos_plan** plan, int n_theta, int n_phi, 
     arkcos_plan* pl = new (std::nothrow) arkcos_plan();
     if (!pl) return ARKCOS_ENOMEM;
     pl->flags = flags; pl->n_table = n_table;
+    pl->m_split = m_split; pl->theta_split = m_split > 0 ? theta_split : 0.0;
     arkcos_status st = ARKCOS_OK;
     try {
         pl->table.assign(k_table, k_table + n_table);

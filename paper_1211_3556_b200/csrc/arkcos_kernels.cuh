@@ -14,7 +14,9 @@ namespace arkcos {
 //   w_ij[d] = A_j * K(gamma_ij(d)),  sin^2(gamma/2) = sin^2((t_i-t_j)/2) + sin t_i sin t_j sin^2(d dphi/2)
 //   (the cancellation-free form of cos(gamma) = cos t_i cos t_j + sin t_i sin t_j cos(d dphi), H3),
 //   K by LINEAR interpolation in the radial table held in shared memory, FP64 throughout, rounded
-//   once to FP32; zero outside the window (so the convolution kernels need no masks).
+//   once to FP32; zero outside the window (so the convolution kernels need no masks).  The table is
+//   uniform in theta, or the paper's two-zone table with half the nodes in the innermost part of the
+//   support (arkcos_plan_create_biased).
 //   One warp per work unit; persistent CTAs so the table is loaded into shared memory once per SM.
 // ================================================================================================
 struct GenParams {
@@ -23,8 +25,11 @@ struct GenParams {
     const double* table;     // [n_table]
     float* weights;
     int n_units, n_phi, n_table;
-    double t_scale;          // (n_table-1)/theta_cut
+    double t_scale;          // (n_table-1)/theta_cut; two-zone table: m_split/theta_split
     int table_in_smem;       // 1: the table was copied to dynamic shared memory
+    int m_split;             // 0: uniform table.  > 0: two-zone table, node m_split at theta_split
+    double theta_split;
+    double t_scale2;         // (n_table-1-m_split)/(theta_cut-theta_split)
 };
 
 constexpr int kGenThreads = 512;
@@ -36,7 +41,8 @@ __device__ __forceinline__ float gen_weight(const GenParams& p, const GenUnit& g
     double h = fma(g.b, p.s2[ad], g.a);
     h = fmin(h, 1.0);
     const double gam = 2.0 * asin(sqrt(h));
-    const double t = gam * p.t_scale;
+    double t = gam * p.t_scale;
+    if (p.m_split > 0 && gam >= p.theta_split) t = (double)p.m_split + (gam - p.theta_split) * p.t_scale2;
     int m = (int)t;
     m = min(m, p.n_table - 2);
     const double f = t - (double)m;

@@ -41,6 +41,16 @@ def table_nodes(theta_cut: float, n_table: int) -> np.ndarray:
     return np.arange(n_table, dtype=np.float64) * (theta_cut / (n_table - 1))
 
 
+def biased_nodes(theta_cut: float, n_table: int, m_split: int, theta_split: float) -> np.ndarray:
+    """Nodes of the paper's two-zone table: node m_split sits at theta_split, the nodes are
+    uniform on [0, theta_split] and on [theta_split, theta_cut].  The paper's choice: m_split = (n-1)/2,
+    theta_split = theta_cut/16.  Where the caller samples K; the lookup itself is the library's and the
+    oracle's own business."""
+    inner = np.arange(m_split + 1, dtype=np.float64) * (theta_split / m_split)
+    outer = theta_split + np.arange(1, n_table - m_split, dtype=np.float64) * ((theta_cut - theta_split) / (n_table - 1 - m_split))
+    return np.concatenate([inner, outer])
+
+
 def gaussian_table(sigma: float, theta_cut: float, n_table: int) -> np.ndarray:
     return gaussian_profile(table_nodes(theta_cut, n_table), sigma)
 

@@ -131,6 +131,12 @@ int main(int argc, char** argv) {
     g.units = s.gen_units.data(); g.s2 = s.s2.data(); g.table = table.data(); g.weights = weights.data();
     g.n_units = (int)s.gen_units.size(); g.n_phi = n_phi; g.n_table = n_table;
     g.t_scale = (double)(n_table - 1) / theta_cut; g.table_in_smem = 1;
+    g.m_split = 0; g.theta_split = 0.0; g.t_scale2 = 0.0;
+    if (const char* e = std::getenv("EMU_M_SPLIT")) {            // two-zone table: EMU_M_SPLIT, EMU_THETA_SPLIT
+        g.m_split = std::atoi(e); g.theta_split = std::atof(std::getenv("EMU_THETA_SPLIT"));
+        g.t_scale = (double)g.m_split / g.theta_split;
+        g.t_scale2 = (double)(n_table - 1 - g.m_split) / (theta_cut - g.theta_split);
+    }
     const int gen_grid = 4;
     emu::g_gridDim = dim3(gen_grid);
     for (int b = 0; b < gen_grid; b++)
