@@ -169,7 +169,7 @@ def workload_config(w: wl.Workload):
 
 
 def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
-            only: str = "all"):
+            only: str = "all", pair_rows: bool = False):
     import torch
     from paper_1211_3556_b200 import arkcos
 
@@ -181,6 +181,8 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     # --only wide|narrow: the library's measurement hook launches one class of work items only (the
     # output is then incomplete; used for per-class timing and ncu captures, never for the bench line)
     flags = {"all": 0, "wide": arkcos.PLAN_ONLY_WIDE, "narrow": arkcos.PLAN_ONLY_NARROW}[only]
+    if pair_rows:                       # experimental paired-rows narrow path (include/arkcos.h)
+        flags |= arkcos.PLAN_PAIR_ROWS
     plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
@@ -305,6 +307,8 @@ def main():
     ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
                     help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
                          "prints a per-class line, not the bench line)")
+    ap.add_argument("--pair-rows", action="store_true",
+                    help="experimental: plan with ARKCOS_PLAN_PAIR_ROWS (paired-rows narrow kernel); noted in config")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = wl.by_name(args.workload)
@@ -325,7 +329,8 @@ def main():
 
     if args.only != "all":
         if rank == 0:
-            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only)
+            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only,
+                          pair_rows=args.pair_rows)
             info = res["info"]
             slots = int(info.fma_slots_wide) if args.only == "wide" else int(info.fma_slots) - int(info.fma_slots_wide)
             peak = res["sm_count"] * FP32_LANES_PER_SM * res["sm_max_mhz"] * 1e6
@@ -336,12 +341,15 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False)
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, pair_rows=args.pair_rows)
     units = float(res["info"].pair_evals) * args.steps
     total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
     if rank == 0:
         cpu = None if (args.no_cpu or world > 1) else cpu_baseline(w, args.cpu_pixels)
-        print(json.dumps(build_line(w, args, res, world, total_ms, total_units, cpu)), flush=True)
+        line = build_line(w, args, res, world, total_ms, total_units, cpu)
+        if args.pair_rows:
+            line["config"]["kernel_variant"] = "experimental paired-rows narrow path (ARKCOS_PLAN_PAIR_ROWS)"
+        print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
     return 0

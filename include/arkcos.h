@@ -58,6 +58,9 @@ typedef enum {
  * rings of the other class are NOT written.  Never set both. */
 #define ARKCOS_PLAN_ONLY_WIDE 4u
 #define ARKCOS_PLAN_ONLY_NARROW 8u
+/* EXPERIMENTAL, not yet measured on a GPU: the paired-rows variant of the NARROW path (the two mirror input rows
+ * i-q, i+q of a ring are processed in one run).  Same results up to FP32 summation order. */
+#define ARKCOS_PLAN_PAIR_ROWS 16u
 
 /*
  * arkcos_plan_create - step S1 (ring-pair scheduler, host FP64) and device uploads.

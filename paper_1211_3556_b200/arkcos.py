@@ -17,6 +17,7 @@ from . import build as _build
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
 PLAN_DEFAULT, PLAN_HOST_ONLY, PLAN_CACHE_WEIGHTS = 0, 1, 2
+PLAN_PAIR_ROWS = 16                          # experimental paired-rows narrow path (include/arkcos.h)
 PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos.h)
 
 _c_plan_p = ctypes.c_void_p

@@ -43,6 +43,7 @@ struct arkcos_plan {
     GenUnit* d_units = nullptr;
     double *d_s2 = nullptr, *d_table = nullptr;
     NarrowRun* d_runs = nullptr;
+    PairRun* d_pair_runs = nullptr;
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging, lazily allocated
     size_t device_bytes = 0;
@@ -84,12 +85,13 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
 arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
-    c.runs = pl->d_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
+    c.runs = pl->d_runs; c.pair_runs = pl->d_pair_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
     c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
     c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
     if (pl->sched.items.empty()) return ARKCOS_OK;
     dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
-    k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
+    if (pl->flags & ARKCOS_PLAN_PAIR_ROWS) k_convolve_pairs<<<grid, kThreads, pl->conv_smem, st>>>(c);
+    else k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
     CU(cudaGetLastError());
     return ARKCOS_OK;
 }
@@ -130,7 +132,7 @@ const char* arkcos_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!pl) return ARKCOS_OK;
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
-        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
+        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_pair_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
         for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
         (void)cudaGetLastError();
@@ -152,7 +154,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
     if (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))) return ARKCOS_EINVAL;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
-    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_PAIR_ROWS)) return ARKCOS_EINVAL;
     if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
     arkcos_plan* pl = new (std::nothrow) arkcos_plan();
@@ -171,7 +173,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
             pl->sm_count = prop.multiProcessorCount;
             if (prop.major < 10) { g_last_cuda_error = "arkcos needs an sm_100 class device"; delete pl; return ARKCOS_EUNSUPPORTED; }
         }
-        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
+        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched, (flags & ARKCOS_PLAN_PAIR_ROWS) != 0);
         if (rc != 0) { delete pl; return (arkcos_status)rc; }
         if (pl->sched.smem_bytes > (size_t)kSmemBudget) { delete pl; return ARKCOS_EUNSUPPORTED; }
         if (flags & (ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) {     // measurement hooks
@@ -189,6 +191,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         if ((st = upload(pl, &pl->d_items, s.items)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_units, s.gen_units)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_runs, s.runs)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_pair_runs, s.pair_runs)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_s2, s.s2)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_table, pl->table)) != ARKCOS_OK) break;
         {
@@ -204,6 +207,9 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         pl->conv_smem = smem;
         if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                      "cudaFuncSetAttribute(k_convolve)")) { st = ARKCOS_ECUDA; break; }
+        if ((flags & ARKCOS_PLAN_PAIR_ROWS) &&
+            !cuda_ok(cudaFuncSetAttribute(k_convolve_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                     "cudaFuncSetAttribute(k_convolve_pairs)")) { st = ARKCOS_ECUDA; break; }
         size_t tab_bytes = (size_t)n_table * sizeof(double);
         pl->table_in_smem = tab_bytes <= 200 * 1024 ? 1 : 0;
         pl->gen_smem = pl->table_in_smem ? tab_bytes : 0;

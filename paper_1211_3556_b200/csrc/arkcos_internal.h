@@ -64,6 +64,16 @@ struct NarrowRun {
     int32_t pad_;
 };
 
+// EXPERIMENTAL (ARKCOS_PLAN_PAIR_ROWS): a run of the paired-rows narrow path.  The two mirror input rows
+// i - q and i + q of a ring have (after taking the union) the same window, so one run slides two register
+// windows over the same taps: twice the FMAs per run start.  Entry e of a ring's list; n = 0 ends the list.
+struct PairRun {
+    int32_t wq_rel_a;   // byte offset of row a's weights in the ring's block, minus 8 * k0
+    int32_t wq_rel_b;   // ... of row b's (paired runs)
+    int32_t k0n;        // k0 | n << 8 | paired << 16
+    int32_t rows;       // row index (0 .. 2R) of a | of b << 8
+};
+
 enum ItemKind : int16_t { kWide = 0, kNarrow = 1 };
 
 // One CTA of the convolution launch.
@@ -103,6 +113,8 @@ struct Schedule {
     std::vector<double> s2;                 // [n_phi/2+1] sin^2(d dphi / 2)
     std::vector<PairDesc> pairs;            // [n_north][2R+1]
     std::vector<NarrowRun> runs;            // [n_north - first_narrow][2R+1]
+    std::vector<PairRun> pair_runs;         // [n_north - first_narrow][2R+1], only with pair_rows
+    bool pair_rows = false;                 // EXPERIMENTAL paired-rows narrow path
     uint32_t narrow_w_base = 0;             // weights of narrow ring i start at narrow_w_base + (i - first_narrow) * narrow_wslot
     std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
     std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows, padded to 4)
@@ -132,6 +144,6 @@ size_t wide_smem_bytes(int R);
 size_t narrow_smem_bytes(int f_log2, int R, int wslot);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out, bool pair_rows = false);
 
 }  // namespace arkcos

@@ -45,12 +45,13 @@ int Schedule::window(int i, int j) const {
     return window_of(*this, i, j);
 }
 
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s) {
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s, bool pair_rows) {
     if (n_theta < 1 || n_phi < 4 || !(theta_cut > 0.0) || !(theta_cut <= kPi * (1.0 + 1e-15))) return 1;
     if (n_phi % 4 != 0) return 4;
     if (sm_count < 1) sm_count = 148;
     s = Schedule();
     s.n_theta = n_theta; s.n_phi = n_phi; s.theta_cut = theta_cut;
+    s.pair_rows = pair_rows;
     s.n_north = (n_theta + 1) / 2;
     const double dtheta = kPi / n_theta, dphi = 2.0 * kPi / n_phi;
     {
@@ -118,17 +119,31 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     };
     s.first_narrow = s.n_north;
     while (s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
+    // stored windows of the narrow rings.  Paired-rows path: the mirror rows i-q, i+q of a ring get the union
+    // of their two windows when it fits [-16, 16) (they differ by a tap at most: D ~ 1/sqrt(sin t_i sin t_j)).
+    std::vector<int> nw_start((size_t)s.n_north * W, 0), nw_ntaps((size_t)s.n_north * W, 0);
+    std::vector<char> nw_paired((size_t)s.n_north * W, 0);
+    for (int i = s.first_narrow; i < s.n_north; i++) {
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (p.half >= 0) narrow_range(p.half, nw_start[(size_t)i * W + r], nw_ntaps[(size_t)i * W + r]);
+        }
+        if (!pair_rows) continue;
+        for (int q = 1; q <= s.R; q++) {
+            const size_t a = (size_t)i * W + (s.R - q), b = (size_t)i * W + (s.R + q);
+            if (s.pairs[a].half < 0 || s.pairs[b].half < 0) continue;
+            const int st = std::min(nw_start[a], nw_start[b]);
+            const int en = std::max(nw_start[a] + nw_ntaps[a], nw_start[b] + nw_ntaps[b]);
+            if (st < -16 || en > 16) continue;
+            nw_start[a] = nw_start[b] = st; nw_ntaps[a] = nw_ntaps[b] = en - st;
+            nw_paired[a] = nw_paired[b] = 1;
+        }
+    }
     {
         unsigned long long wslot = 0;
         for (int i = s.first_narrow; i < s.n_north; i++) {
             unsigned long long slots = 0;
-            for (int r = 0; r < W; r++) {
-                const PairDesc& p = s.pairs[(size_t)i * W + r];
-                if (p.half < 0) continue;
-                int start, ntaps;
-                narrow_range(p.half, start, ntaps);
-                slots += (unsigned long long)ntaps;
-            }
+            for (int r = 0; r < W; r++) slots += (unsigned long long)nw_ntaps[(size_t)i * W + r];
             wslot = std::max(wslot, slots);
         }
         s.narrow_wslot = (int)((wslot + 3) & ~3ull);
@@ -155,7 +170,8 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         for (int r = 0; r < W; r++) {
             PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half < 0) continue;
-            if (wide) wide_range(p.half, p.start, p.ntaps); else narrow_range(p.half, p.start, p.ntaps);
+            if (wide) wide_range(p.half, p.start, p.ntaps);
+            else { p.start = nw_start[(size_t)i * W + r]; p.ntaps = nw_ntaps[(size_t)i * W + r]; }
             const unsigned long long floats = (unsigned long long)p.ntaps;
             if (w_off + floats > 0xFFFFFFF0ull) return 4;
             p.w_off = (uint32_t)w_off;
@@ -178,6 +194,23 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             u.n = p.ntaps / 2;
             u.wq_rel = 4 * (int32_t)(p.w_off - s.ring_w_off[i]) - 8 * u.k0;
         }
+    if (pair_rows) {
+        s.pair_runs.assign((size_t)(s.n_north - s.first_narrow) * W, PairRun{0, 0, 0, 0});
+        for (int i = s.first_narrow; i < s.n_north; i++) {
+            PairRun* list = &s.pair_runs[(size_t)(i - s.first_narrow) * W];
+            int e = 0;
+            auto rel = [&](int r, int k0) { return 4 * (int32_t)(s.pairs[(size_t)i * W + r].w_off - s.ring_w_off[i]) - 8 * k0; };
+            for (int r = 0; r < W; r++) {
+                const PairDesc& p = s.pairs[(size_t)i * W + r];
+                if (p.ntaps == 0) continue;
+                const bool paired = nw_paired[(size_t)i * W + r] != 0;
+                if (paired && r > s.R) continue;                        // emitted with its mirror row
+                const int k0 = (kHaloNarrow + p.start) / 2, n = p.ntaps / 2;
+                const int rb = paired ? 2 * s.R - r : r;
+                list[e++] = PairRun{rel(r, k0), rel(rb, k0), k0 | (n << 8) | ((paired ? 1 : 0) << 16), r | (rb << 8)};
+            }
+        }
+    }
 
     // ---- generator work units: one warp writes up to kGenUnitTaps taps (steps) of one ring pair -----
     for (int i = 0; i < s.n_north; i++) {

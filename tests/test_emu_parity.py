@@ -35,13 +35,13 @@ def emu_bin():
     return EMU_BIN
 
 
-def emulate(emu, tmp_path, x32, table, theta_cut, only=None):
+def emulate(emu, tmp_path, x32, table, theta_cut, only=None, env=None):
     n_theta, n_phi = x32.shape
     t, i, o = (str(tmp_path / n) for n in ("table.f64", "in.f32", "out.f32"))
     np.ascontiguousarray(table, dtype=np.float64).tofile(t)
     np.ascontiguousarray(x32, dtype=np.float32).tofile(i)
     cmd = [emu, str(n_theta), str(n_phi), repr(float(theta_cut)), str(table.size), t, i, o] + ([only] if only else [])
-    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=dict(os.environ, **(env or {})))
     assert res.returncode == 0, (res.stdout + res.stderr)[-3000:]
     return np.fromfile(o, dtype=np.float32).reshape(n_theta, n_phi).astype(np.float64), res.stdout
 
@@ -86,6 +86,22 @@ def test_emulated_two_phi_tiles_and_oscillating_kernel(emu_bin, tmp_path):
     table = np.cos(7.0 * th / cut) * np.exp(-0.5 * (th / (0.4 * cut)) ** 2) * 50.0
     x32 = np.random.default_rng(7).standard_normal((n_theta, n_phi)).astype(np.float32)
     got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    expect = oracle.convolve(x32, table, cut, level=1)
+    rms = math.sqrt((expect ** 2).mean())
+    assert not np.isnan(got).any(), log
+    assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("n_theta,n_phi,sigma_deg,cut_sigmas", [(64, 128, 3.0, 3.0), (200, 512, 1.27, 3.0), (301, 256, 0.9, 4.1)])
+def test_emulated_paired_rows_path(emu_bin, tmp_path, n_theta, n_phi, sigma_deg, cut_sigmas):
+    """EXPERIMENTAL ARKCOS_PLAN_PAIR_ROWS kernel (k_convolve_pairs): mirror rows i-q, i+q in one run."""
+    import re
+    sigma = math.radians(sigma_deg)
+    cut = cut_sigmas * sigma
+    table = gaussian_table(sigma, cut, 1024)
+    x32 = np.random.default_rng(2000 + n_theta).standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut, env={"EMU_PAIR_ROWS": "1"})
+    assert int(re.search(r"paired runs (\d+)", log).group(1)) > 0, log      # the paired chain really ran
     expect = oracle.convolve(x32, table, cut, level=1)
     rms = math.sqrt((expect ** 2).mean())
     assert not np.isnan(got).any(), log
