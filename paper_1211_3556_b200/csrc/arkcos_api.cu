@@ -200,7 +200,10 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
             if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); st = ARKCOS_ENOMEM; break; }
             if (!cuda_ok(e, "cudaMalloc(weights)")) { st = ARKCOS_ECUDA; break; }
             pl->device_bytes += bytes;
-            if (!cuda_ok(cudaMemset(pl->d_weights, 0, bytes), "cudaMemset(weights)")) { st = ARKCOS_ECUDA; break; }
+            // gaps between ring blocks and window padding stay zero for the life of the plan.  The memset runs on
+            // the legacy default stream, which non-blocking user streams do not wait for: finish it here.
+            if (!cuda_ok(cudaMemset(pl->d_weights, 0, bytes), "cudaMemset(weights)") ||
+                !cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize(weights)")) { st = ARKCOS_ECUDA; break; }
         }
         // launch configuration
         const size_t smem = s.smem_bytes;
