@@ -7,7 +7,8 @@
 // Shared memory is a heap block of exactly the launch's dynamic size (AddressSanitizer sees overruns),
 // every ld.shared wrapper checks bounds and alignment, every cp.async source must lie in a registered
 // global buffer.  Shared memory and the output start as NaN, so a value consumed before it was staged
-// shows up in the result.
+// shows up in the result.  EMU_EAGER=1 performs cp.async copies at issue instead of at the wait, which exposes
+// a copy that lands in a buffer still being read.
 //
 //   emu_arkcos n_theta n_phi theta_cut n_table table.f64 in.f32 out.f32 [only_wide|only_narrow]
 //
@@ -51,9 +52,14 @@ void check_global(const void* p, size_t bytes) {
 struct Pending { uint32_t dst; const void* src; };
 static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
 static thread_local std::vector<Pending> t_open;                  // not yet committed
+// Two modes bracket what the hardware may do with a cp.async: DEFERRED (default) performs the copy only at
+// the wait - a read before the wait sees stale data (RAW hazard); EAGER (EMU_EAGER=1) performs it at once - a
+// copy into a buffer that other threads still read clobbers it (WAR hazard).
+static const bool g_eager = std::getenv("EMU_EAGER") != nullptr;
 void cp_async_enqueue(uint32_t dst, const void* src) {
     (void)smem_at(dst, 16);
     check_global(src, 16);
+    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); return; }
     t_open.push_back(Pending{dst, src});
 }
 void cp_async_commit_group() { t_groups.push_back(std::move(t_open)); t_open.clear(); }

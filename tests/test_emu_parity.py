@@ -61,6 +61,24 @@ CASES = [
 ]
 
 
+@pytest.mark.parametrize("pair_rows", [False, True])
+def test_emulated_eager_cp_async(emu_bin, tmp_path, pair_rows):
+    """cp.async copies performed at issue (EMU_EAGER): a copy into a row slot, weight block or stage buffer that is
+    still being read would corrupt the result.  Several narrow passes and multi-stage wide rows."""
+    n_theta, n_phi, sigma = 200, 512, math.radians(1.27)
+    cut = 3.0 * sigma
+    table = gaussian_table(sigma, cut, 1024)
+    x32 = np.random.default_rng(31).standard_normal((n_theta, n_phi)).astype(np.float32)
+    env = {"EMU_EAGER": "1"}
+    if pair_rows:
+        env["EMU_PAIR_ROWS"] = "1"
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut, env=env)
+    expect = oracle.convolve(x32, table, cut, level=1)
+    rms = math.sqrt((expect ** 2).mean())
+    assert not np.isnan(got).any(), log
+    assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
+
+
 @pytest.mark.parametrize("n_theta,n_phi,sigma_deg,cut_sigmas", CASES)
 def test_emulated_kernels_match_oracle(emu_bin, tmp_path, n_theta, n_phi, sigma_deg, cut_sigmas):
     sigma = math.radians(sigma_deg)
