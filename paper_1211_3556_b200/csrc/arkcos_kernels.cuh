@@ -63,9 +63,16 @@ __global__ void __launch_bounds__(kGenThreads) k_generate_weights(const GenParam
         tab = s_table;
     }
     const int warps = kGenThreads / 32, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int u = blockIdx.x * warps + warp; u < p.n_units; u += gridDim.x * warps) {
-        const GenUnit g = p.units[u];
+    // the next unit's descriptor is fetched while the current unit is computed (a warp handles ~20 units
+    // one after the other; each descriptor would otherwise cost a full global-memory round trip)
+    const int stride = gridDim.x * warps;
+    int u = blockIdx.x * warps + warp;
+    if (u >= p.n_units) return;
+    GenUnit g = p.units[u];
+    for (; u < p.n_units; u += stride) {
+        const GenUnit nxt = p.units[u + stride < p.n_units ? u + stride : u];
         for (int e = lane; e < g.count; e += 32) p.weights[(size_t)g.w_base + e] = gen_weight(p, g, tab, g.d0 + e);
+        g = nxt;
     }
 }
 
