@@ -48,18 +48,20 @@ def load_peaks():
 
 
 def ncu_traffic(workload: str):
-    """dram bytes per launch of the convolution kernel from the committed ncu capture, or None."""
+    """(dram bytes per launch of k_convolve, capture id) from the ncu `--set full` capture of THIS round's kernel
+    committed as profiles/dram_traffic.csv (rows: workload, kernel, bytes, capture), or (None, None).  A row is
+    only ever written from a capture named beside it in profiles/; it is never typed in from an older kernel."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return None, None
     for line in open(path):
         parts = [p.strip() for p in line.split(",")]
-        if len(parts) >= 3 and parts[0] == workload and parts[1] == "k_convolve":
+        if len(parts) >= 4 and parts[0] == workload and parts[1] == "k_convolve":
             try:
-                return float(parts[2])
+                return float(parts[2]), parts[3]
             except ValueError:
-                return None
-    return None
+                return None, None
+    return None, None
 
 
 class ClockSampler:
@@ -163,13 +165,15 @@ def workload_config(w: wl.Workload):
     return {"workload": w.name, "n_theta": w.n_theta, "n_phi": w.n_phi,
             "theta_cut_arcmin": w.theta_cut / wl.ARCMIN, "kernel": w.kernel,
             "fwhm_arcmin": w.sigma / wl.FWHM_TO_SIGMA / wl.ARCMIN, "n_table": w.n_table,
-            "maps_per_step": 1, "parallelism": "replicas (no sharding, SURVEY 8(e))",
-            "l2": "map in+out = %.0f MB per step vs 126 MB L2: %s" % (
-                8e-6 * w.n_pix, "larger than L2, no flush needed" if 8 * w.n_pix > 126e6 else "input buffers rotated")}
+            "maps_per_step": len(w.map_seeds), "parallelism": "replicas (no sharding, SURVEY 8(e))",
+            "l2": "maps in+out = %.0f MB per step vs 126 MB L2: %s" % (
+                8e-6 * w.n_pix * len(w.map_seeds),
+                "larger than L2, no flush needed" if 8 * w.n_pix * len(w.map_seeds) > 126e6 else "input buffers rotated")}
 
 
 def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
-            only: str = "all", pair_rows: bool = False):
+            only: str = "all"):
+    """One step = S2 + S3 over ALL maps of the workload (configs[4]: the batch of 8 through arkcos_convolve_batch)."""
     import torch
     from paper_1211_3556_b200 import arkcos
 
@@ -177,23 +181,22 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     dev = torch.device("cuda", local_rank)
     hbm_gbs, sm_max_mhz, peak_src = load_peaks()
     table = w.table()
-    x32 = w.map_f32()
+    n_maps = len(w.map_seeds)
+    x32 = np.stack([w.map_f32(m) for m in range(n_maps)]) if n_maps > 1 else w.map_f32()
     # --only wide|narrow: the library's measurement hook launches one class of work items only (the
     # output is then incomplete; used for per-class timing and ncu captures, never for the bench line)
     flags = {"all": 0, "wide": arkcos.PLAN_ONLY_WIDE, "narrow": arkcos.PLAN_ONLY_NARROW}[only]
-    if pair_rows:                       # experimental paired-rows narrow path (include/arkcos.h)
-        flags |= arkcos.PLAN_PAIR_ROWS
     plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
     sh = stream.cuda_stream
     # rotate input buffers when the map would otherwise sit in L2 between steps
-    n_rot = 1 if 8 * w.n_pix > 126e6 else max(2, int(math.ceil(260e6 / (4 * w.n_pix))))
+    n_rot = 1 if 8 * w.n_pix * n_maps > 126e6 else max(2, int(math.ceil(260e6 / (4 * w.n_pix))))
     d_in = [torch.from_numpy(x32).to(dev) for _ in range(n_rot)]
     d_out = torch.empty_like(d_in[0])
     with torch.cuda.stream(stream):
         for i in range(warmup):
-            plan.convolve(d_in[i % n_rot], d_out, sh)
+            plan.convolve_batch(d_in[i % n_rot], d_out, n_maps, sh)
     stream.synchronize()
 
     # ---- timed region: K back-to-back steps, CUDA events on the launching stream --------------------
@@ -206,7 +209,7 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     with torch.cuda.stream(stream):
         e0.record(stream)
         for i in range(steps):
-            plan.convolve(d_in[i % n_rot], d_out, sh)
+            plan.convolve_batch(d_in[i % n_rot], d_out, n_maps, sh)
         e1.record(stream)
     stream.synchronize()
     torch.cuda.synchronize()
@@ -215,14 +218,15 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     # ---- per-kernel device times (CUDA events inside the library, same stream), K more steps --------
     gen_ms, conv_ms = [], []
     for i in range(steps):
-        g, c = plan.convolve_timed(d_in[i % n_rot], d_out, sh)
+        g, c = plan.measure_convolve(d_in[i % n_rot], d_out, sh, n_maps)
         gen_ms.append(g); conv_ms.append(c)
     clocks = sampler.stop()
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
     if want_e2e:
-        h_in = torch.from_numpy(x32).pin_memory()
+        plan.reserve_host_io()
+        h_in = torch.from_numpy(x32[0] if n_maps > 1 else x32).pin_memory()
         h_out = torch.empty_like(h_in).pin_memory()
         hi, ho = h_in.numpy(), h_out.numpy()
         for _ in range(min(warmup, 2)):
@@ -239,7 +243,7 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
 
     result = {"elapsed_ms": elapsed_ms, "gen_ms": float(np.mean(gen_ms)), "conv_ms": float(np.mean(conv_ms)),
               "conv_ms_min": float(np.min(conv_ms)), "clocks": clocks, "info": info, "e2e": e2e,
-              "hbm_gbs": hbm_gbs, "sm_max_mhz": sm_max_mhz, "peak_src": peak_src,
+              "hbm_gbs": hbm_gbs, "sm_max_mhz": sm_max_mhz, "peak_src": peak_src, "n_maps": n_maps,
               "device_name": torch.cuda.get_device_name(dev), "sm_count": info.sm_count}
     plan.destroy()
     return result
@@ -247,28 +251,30 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
 
 def build_line(w, args, res, world, total_ms, total_units, cpu):
     info = res["info"]
-    pair_evals = int(info.pair_evals)
+    n_maps = res["n_maps"]
+    pair_evals = int(info.pair_evals) * n_maps          # per step (= per launch of k_convolve)
     ms_per_step = total_ms / args.steps
     value = replicas.throughput(total_units, total_ms)
     peak_tflops = res["sm_count"] * FP32_LANES_PER_SM * 2 * res["sm_max_mhz"] * 1e6 / 1e12
     achieved_tflops = 2.0 * pair_evals / (res["conv_ms"] * 1e-3) / 1e12
-    hbm_achieved = 8.0 * w.n_pix / (res["conv_ms"] * 1e-3) / 1e9
+    hbm_achieved = 8.0 * w.n_pix * n_maps / (res["conv_ms"] * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic(w.name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": workload_config(w),
-        "output_pixels_per_s": world * w.n_pix * args.steps / (total_ms * 1e-3),
-        "pair_evals_per_map": pair_evals,
+        "output_pixels_per_s": world * w.n_pix * n_maps * args.steps / (total_ms * 1e-3),
+        "pair_evals_per_map": int(info.pair_evals),
         "kernel_ms": {"generate_weights": res["gen_ms"], "convolve": res["conv_ms"], "convolve_min": res["conv_ms_min"]},
         "roofline": {
             "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": achieved_tflops / peak_tflops, "traffic": ncu_traffic(w.name),
+            "frac": achieved_tflops / peak_tflops, "traffic": traffic, "traffic_source": traffic_src,
             "kernel": "k_convolve", "flops_per_launch": 2.0 * pair_evals,
             "peak_source": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json)" % (
                 res["sm_count"], res["sm_max_mhz"], res["peak_src"]),
-            "issued_lane_frac": float(info.fma_slots) / (res["conv_ms"] * 1e-3) / (peak_tflops * 1e12 / 2.0),
+            "issued_lane_frac": float(info.fma_slots) * n_maps / (res["conv_ms"] * 1e-3) / (peak_tflops * 1e12 / 2.0),
             "hbm": {"achieved": hbm_achieved, "peak": res["hbm_gbs"], "unit": "GB/s", "frac": hbm_achieved / res["hbm_gbs"],
-                    "algorithmic_bytes_per_launch": 8.0 * w.n_pix},
+                    "algorithmic_bytes_per_launch": 8.0 * w.n_pix * n_maps},
         },
         "clocks": res["clocks"],
         "gpu_launches": args.steps * int(info.kernels_per_convolve),
@@ -276,7 +282,7 @@ def build_line(w, args, res, world, total_ms, total_units, cpu):
     }
     if res["e2e"] is not None:
         e = res["e2e"]
-        line["e2e"] = {"value": world * pair_evals / (e["ms_per_step"] * 1e-3), "unit": UNIT,
+        line["e2e"] = {"value": world * int(info.pair_evals) / (e["ms_per_step"] * 1e-3), "unit": UNIT, "maps_per_step": 1,
                        "h2d_bytes_per_step": 4 * w.n_pix, "d2h_bytes_per_step": 4 * w.n_pix,
                        "ms_per_step": e["ms_per_step"], "steps": e["steps"], "host_memory": "pinned",
                        "api": "arkcos_convolve_host"}
@@ -287,7 +293,7 @@ def build_line(w, args, res, world, total_ms, total_units, cpu):
 
 def cpu_baseline(w: wl.Workload, n_pixels: int):
     pairs, dt, cores = oracle_sample(w, n_pixels, 4242)
-    return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+    return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "tuned": False,
             "sample": f"{n_pixels} seeded uniform random output pixels of {w.name} ({pairs} pair evals in {dt:.1f} s), "
                       "oracle level 1, OpenMP dynamic",
             "output_pixels_per_s": n_pixels / dt}
@@ -307,8 +313,6 @@ def main():
     ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
                     help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
                          "prints a per-class line, not the bench line)")
-    ap.add_argument("--pair-rows", action="store_true",
-                    help="experimental: plan with ARKCOS_PLAN_PAIR_ROWS (paired-rows narrow kernel); noted in config")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = wl.by_name(args.workload)
@@ -329,10 +333,10 @@ def main():
 
     if args.only != "all":
         if rank == 0:
-            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only,
-                          pair_rows=args.pair_rows)
+            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only)
             info = res["info"]
             slots = int(info.fma_slots_wide) if args.only == "wide" else int(info.fma_slots) - int(info.fma_slots_wide)
+            slots *= res["n_maps"]
             peak = res["sm_count"] * FP32_LANES_PER_SM * res["sm_max_mhz"] * 1e6
             print(json.dumps({"report": "class_only", "only": args.only, "workload": w.name, "items": int(info.n_items),
                               "convolve_ms": res["conv_ms"], "fma_slots": slots,
@@ -341,14 +345,12 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, pair_rows=args.pair_rows)
-    units = float(res["info"].pair_evals) * args.steps
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False)
+    units = float(res["info"].pair_evals) * res["n_maps"] * args.steps
     total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
     if rank == 0:
         cpu = None if (args.no_cpu or world > 1) else cpu_baseline(w, args.cpu_pixels)
         line = build_line(w, args, res, world, total_ms, total_units, cpu)
-        if args.pair_rows:
-            line["config"]["kernel_variant"] = "experimental paired-rows narrow path (ARKCOS_PLAN_PAIR_ROWS)"
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -362,11 +364,11 @@ def sweep(args):
     for w in wl.all_workloads():
         res = measure(w, max(3, args.steps // 2), 3, None, 0, want_cpu=False, want_e2e=False)
         a = argparse.Namespace(**vars(args)); a.steps = max(3, args.steps // 2)
-        line = build_line(w, a, res, 1, res["elapsed_ms"], float(res["info"].pair_evals) * a.steps, None)
+        line = build_line(w, a, res, 1, res["elapsed_ms"], float(res["info"].pair_evals) * res["n_maps"] * a.steps, None)
         line["report"] = "sweep"
         print(json.dumps(line), flush=True)
         key = w.name.split("_cut")[0]
-        curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"]))
+        curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"] / res["n_maps"]))
     for key, pts in curve.items():
         if len(pts) < 3:
             continue

@@ -39,7 +39,9 @@ typedef enum {
     ARKCOS_EINVAL = 1,       /* bad argument (range, NULL, alignment, aliasing, non-finite table) */
     ARKCOS_ENOMEM = 2,       /* host or device allocation failed                                  */
     ARKCOS_ECUDA = 3,        /* a CUDA runtime call failed (no device, launch error, ...)         */
-    ARKCOS_EUNSUPPORTED = 4  /* valid request this build cannot serve (e.g. n_phi % 4 != 0)       */
+    ARKCOS_EUNSUPPORTED = 4, /* valid request this build cannot serve (e.g. n_phi % 4 != 0)       */
+    ARKCOS_EINTERNAL = 5     /* the ring-pair schedule failed its own validation (a bug in this   */
+                             /* library; nothing was uploaded or launched)                        */
 } arkcos_status;
 
 /* flags of arkcos_plan_create_ex */
@@ -49,18 +51,9 @@ typedef enum {
 #define ARKCOS_PLAN_HOST_ONLY 1u
 /* Run the weight generator (step S2) once, at plan creation, and reuse its output in every
  * arkcos_convolve.  Default is to regenerate the weights on the fly inside each call
- * (north_star (b)); both give bit-identical results.  Cached plans may be used from several
- * streams concurrently; on-the-fly plans rewrite the (identical) weights in each call and must not
- * be used from two streams at the same time. */
+ * (north_star (b)); both give bit-identical results. */
 #define ARKCOS_PLAN_CACHE_WEIGHTS 2u
-/* Measurement hooks: launch only the WIDE (polar / high-latitude rings) or only the NARROW
- * (equatorial band) work items of step S3, to time the two kernel paths separately.  The output
- * rings of the other class are NOT written.  Never set both. */
-#define ARKCOS_PLAN_ONLY_WIDE 4u
-#define ARKCOS_PLAN_ONLY_NARROW 8u
-/* EXPERIMENTAL, not yet measured on a GPU: the paired-rows variant of the NARROW path (the two mirror input rows
- * i-q, i+q of a ring are processed in one run).  Same results up to FP32 summation order. */
-#define ARKCOS_PLAN_PAIR_ROWS 16u
+/* (bits 4 and 8 are measurement hooks declared in arkcos_measure.h) */
 
 /*
  * arkcos_plan_create - step S1 (ring-pair scheduler, host FP64) and device uploads.
@@ -70,8 +63,11 @@ typedef enum {
  *                  both ends included; copied; must be finite
  *   n_table        >= 2
  *   theta_cut_rad  support radius, 0 < theta_cut <= pi, inclusive (K_real(theta <= theta_cut))
- * The plan owns its device memory on the device current at this call.
- * Errors: EINVAL, EUNSUPPORTED (n_phi % 4 != 0), ENOMEM, ECUDA.
+ * The plan owns its device memory on the device current at this call.  Before anything is uploaded the
+ * schedule is validated on the host: every global range and shared-memory offset the kernels will form from
+ * it is re-derived and bounds-checked (EINTERNAL if not; the kernels themselves carry no bounds checks).
+ * All uploads have completed when the call returns, so the plan may be used at once on any stream.
+ * Errors: EINVAL, EUNSUPPORTED (n_phi % 4 != 0), ENOMEM, ECUDA, EINTERNAL.
  */
 arkcos_status arkcos_plan_create(arkcos_plan **plan, int n_theta, int n_phi, const double *k_table,
                                  int n_table, double theta_cut_rad);
@@ -102,7 +98,13 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan **plan, int n_theta, int n_p
  *   d_out  DEVICE, same shape, 16-byte aligned, fully overwritten; must not overlap d_in
  *   stream cudaStream_t cast to void* (NULL = legacy default stream)
  * Asynchronous on `stream`: no allocation, no host synchronisation, no host<->device copy.
- * Errors: EINVAL (NULL / misaligned / overlapping pointers), EUNSUPPORTED (host-only plan), ECUDA.
+ * A plan is immutable and may be used from several streams and host threads at the same time: the only
+ * plan-owned memory a call writes is the weight buffer, and step S2 is a pure function of the plan - every
+ * call rewrites each weight with the bit-identical value, and each call's own S2 precedes its own S3 on its
+ * stream, so concurrent calls never observe a different value (cached plans do not write at all).
+ * The current device must be the plan's device.
+ * Errors: EINVAL (NULL / misaligned / overlapping pointers, wrong current device), EUNSUPPORTED (host-only
+ * plan), ECUDA.
  */
 arkcos_status arkcos_convolve(const arkcos_plan *plan, const float *d_in, float *d_out, void *stream);
 
@@ -115,11 +117,14 @@ arkcos_status arkcos_convolve_batch(const arkcos_plan *plan, const float *d_in, 
                                     void *stream);
 
 /*
- * arkcos_convolve_host - end-to-end convenience: HOST map in, HOST map out.
- * Copies h_in to a plan-owned device buffer (allocated on first use), runs arkcos_convolve and
- * copies the result back; returns after the result is in h_out (synchronises `stream`).
- * Pinned host memory makes the copies asynchronous DMA; pageable memory also works.
+ * arkcos_convolve_host - end to end: HOST map in, HOST map out.
+ * Copies h_in to plan-owned device staging, runs arkcos_convolve and copies the result back; returns after
+ * the result is in h_out (synchronises `stream`).  Pinned host memory makes the copies asynchronous DMA;
+ * pageable memory also works.  The staging (two maps) is allocated by arkcos_plan_reserve_host_io, which this
+ * call makes itself if the caller has not; unlike arkcos_convolve it uses plan-owned staging, so one call per
+ * plan at a time.
  */
+arkcos_status arkcos_plan_reserve_host_io(arkcos_plan *plan);
 arkcos_status arkcos_convolve_host(arkcos_plan *plan, const float *h_in, float *h_out, void *stream);
 
 /* Releases the plan and its device memory.  NULL is a no-op. */
@@ -176,14 +181,6 @@ arkcos_status arkcos_plan_window(const arkcos_plan *plan, int i, int j, int *hal
  * Synchronises the device.  EUNSUPPORTED on host-only plans.
  */
 arkcos_status arkcos_plan_pair_weights(const arkcos_plan *plan, int i, int j, float *h_w, int cap, int *n);
-
-/*
- * Measurement hook: one arkcos_convolve on `stream` with CUDA events around each kernel;
- * synchronises the stream and returns the device time of the weight generator (0 for cached plans)
- * and of the convolution kernel(s), in milliseconds.
- */
-arkcos_status arkcos_convolve_timed(const arkcos_plan *plan, const float *d_in, float *d_out, void *stream,
-                                    float *ms_generate, float *ms_convolve);
 
 #ifdef __cplusplus
 }

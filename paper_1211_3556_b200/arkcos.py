@@ -15,10 +15,9 @@ import numpy as np
 
 from . import build as _build
 
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, EINTERNAL = 0, 1, 2, 3, 4, 5
 PLAN_DEFAULT, PLAN_HOST_ONLY, PLAN_CACHE_WEIGHTS = 0, 1, 2
-PLAN_PAIR_ROWS = 16                          # experimental paired-rows narrow path (include/arkcos.h)
-PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos.h)
+PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos_measure.h)
 
 _c_plan_p = ctypes.c_void_p
 
@@ -44,7 +43,7 @@ class ArkcosError(RuntimeError):
 
 _lib = None
 
-# every symbol include/arkcos.h declares: (name, restype, argtypes)
+# every symbol include/arkcos.h and include/arkcos_measure.h declare: (name, restype, argtypes)
 SYMBOLS = [
     ("arkcos_plan_create", ctypes.c_int, [ctypes.POINTER(_c_plan_p), ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                           ctypes.c_int, ctypes.c_double]),
@@ -55,6 +54,7 @@ SYMBOLS = [
     ("arkcos_convolve", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     ("arkcos_convolve_batch", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     ("arkcos_convolve_host", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    ("arkcos_plan_reserve_host_io", ctypes.c_int, [_c_plan_p]),
     ("arkcos_plan_destroy", ctypes.c_int, [_c_plan_p]),
     ("arkcos_status_string", ctypes.c_char_p, [ctypes.c_int]),
     ("arkcos_last_cuda_error", ctypes.c_char_p, []),
@@ -64,8 +64,10 @@ SYMBOLS = [
     ("arkcos_plan_window", ctypes.c_int, [_c_plan_p, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
     ("arkcos_plan_pair_weights", ctypes.c_int, [_c_plan_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int,
                                                 ctypes.POINTER(ctypes.c_int)]),
-    ("arkcos_convolve_timed", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
-                                             ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
+    ("arkcos_measure_convolve", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
+                                               ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
+    ("arkcos_plan_validate", ctypes.c_int, [_c_plan_p, ctypes.c_char_p, ctypes.c_int]),
+    ("arkcos_plan_item", ctypes.c_int, [_c_plan_p, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
 ]
 
 
@@ -131,11 +133,28 @@ class Plan:
     def convolve_host(self, h_in, h_out, stream: int = 0):
         _check(lib().arkcos_convolve_host(self._h, _ptr(h_in), _ptr(h_out), stream), "arkcos_convolve_host")
 
-    def convolve_timed(self, d_in, d_out, stream: int = 0) -> Tuple[float, float]:
+    def reserve_host_io(self):
+        _check(lib().arkcos_plan_reserve_host_io(self._h), "arkcos_plan_reserve_host_io")
+
+    def measure_convolve(self, d_in, d_out, stream: int = 0, n_maps: int = 1) -> Tuple[float, float]:
         a, b = ctypes.c_float(0), ctypes.c_float(0)
-        _check(lib().arkcos_convolve_timed(self._h, _ptr(d_in), _ptr(d_out), stream, ctypes.byref(a), ctypes.byref(b)),
-               "arkcos_convolve_timed")
+        _check(lib().arkcos_measure_convolve(self._h, _ptr(d_in), _ptr(d_out), int(n_maps), stream, ctypes.byref(a), ctypes.byref(b)),
+               "arkcos_measure_convolve")
         return float(a.value), float(b.value)
+
+    def items(self):
+        """[(kind, ring, nrings, k0, n_out_phi, splits)] of the convolution launch (arkcos_plan_item)."""
+        out = []
+        f = (ctypes.c_int * 6)()
+        for k in range(self.info().n_items):
+            _check(lib().arkcos_plan_item(self._h, k, f), "arkcos_plan_item")
+            out.append(tuple(int(v) for v in f))
+        return out
+
+    def validate(self) -> Tuple[int, str]:
+        buf = ctypes.create_string_buffer(256)
+        status = lib().arkcos_plan_validate(self._h, buf, 256)
+        return int(status), buf.value.decode()
 
     # -- introspection ------------------------------------------------------------------------
     def work(self) -> Tuple[int, int, int]:

@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "../../include/arkcos.h"
+#include "../../include/arkcos_measure.h"
 #include "arkcos_internal.h"
 #include "arkcos_kernels.cuh"
 
@@ -43,13 +44,11 @@ struct arkcos_plan {
     GenUnit* d_units = nullptr;
     double *d_s2 = nullptr, *d_table = nullptr;
     NarrowRun* d_runs = nullptr;
-    PairRun* d_pair_runs = nullptr;
     float* d_weights = nullptr;
-    float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging, lazily allocated
+    float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging (arkcos_plan_reserve_host_io)
     size_t device_bytes = 0;
     size_t conv_smem = 0, gen_smem = 0;
     int gen_grid = 0, table_in_smem = 0;
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -85,13 +84,12 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
 arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
-    c.runs = pl->d_runs; c.pair_runs = pl->d_pair_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
+    c.runs = pl->d_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
     c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
     c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
     if (pl->sched.items.empty()) return ARKCOS_OK;
     dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
-    if (pl->flags & ARKCOS_PLAN_PAIR_ROWS) k_convolve_pairs<<<grid, kThreads, pl->conv_smem, st>>>(c);
-    else k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
+    k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
     CU(cudaGetLastError());
     return ARKCOS_OK;
 }
@@ -99,6 +97,9 @@ arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d
 arkcos_status check_io(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps) {
     if (!pl || !d_in || !d_out || n_maps < 1) return ARKCOS_EINVAL;
     if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return ARKCOS_ECUDA;
+    if (dev != pl->device) return ARKCOS_EINVAL;                // the plan's memory lives on another device
     if (((uintptr_t)d_in & 15u) || ((uintptr_t)d_out & 15u)) return ARKCOS_EINVAL;
     const size_t bytes = (size_t)n_maps * pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
     const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
@@ -123,6 +124,7 @@ const char* arkcos_status_string(arkcos_status s) {
         case ARKCOS_ENOMEM: return "ARKCOS_ENOMEM: out of memory";
         case ARKCOS_ECUDA: return "ARKCOS_ECUDA: CUDA runtime error";
         case ARKCOS_EUNSUPPORTED: return "ARKCOS_EUNSUPPORTED: not supported by this build";
+        case ARKCOS_EINTERNAL: return "ARKCOS_EINTERNAL: the schedule failed its own validation";
     }
     return "ARKCOS_?: unknown status";
 }
@@ -132,9 +134,8 @@ const char* arkcos_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!pl) return ARKCOS_OK;
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
-        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_pair_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
+        cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
-        for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
         (void)cudaGetLastError();
     }
     delete pl;
@@ -154,7 +155,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
     if (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))) return ARKCOS_EINVAL;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
-    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_PAIR_ROWS)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
     arkcos_plan* pl = new (std::nothrow) arkcos_plan();
@@ -173,7 +174,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
             pl->sm_count = prop.multiProcessorCount;
             if (prop.major < 10) { g_last_cuda_error = "arkcos needs an sm_100 class device"; delete pl; return ARKCOS_EUNSUPPORTED; }
         }
-        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched, (flags & ARKCOS_PLAN_PAIR_ROWS) != 0);
+        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
         if (rc != 0) { delete pl; return (arkcos_status)rc; }
         if (pl->sched.smem_bytes > (size_t)kSmemBudget) { delete pl; return ARKCOS_EUNSUPPORTED; }
         if (flags & (ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) {     // measurement hooks
@@ -191,7 +192,6 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         if ((st = upload(pl, &pl->d_items, s.items)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_units, s.gen_units)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_runs, s.runs)) != ARKCOS_OK) break;
-        if ((st = upload(pl, &pl->d_pair_runs, s.pair_runs)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_s2, s.s2)) != ARKCOS_OK) break;
         if ((st = upload(pl, &pl->d_table, pl->table)) != ARKCOS_OK) break;
         {
@@ -205,26 +205,20 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
             if (!cuda_ok(cudaMemset(pl->d_weights, 0, bytes), "cudaMemset(weights)") ||
                 !cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize(weights)")) { st = ARKCOS_ECUDA; break; }
         }
-        // launch configuration
-        const size_t smem = s.smem_bytes;
-        pl->conv_smem = smem;
-        if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+        // launch configuration.  The dynamic shared-memory limit is an attribute of the KERNEL, shared by every
+        // plan of the process: always set it to the library's maximum, never to this plan's own size (a later,
+        // smaller plan must not lower it under an earlier plan's launches).
+        pl->conv_smem = s.smem_bytes;
+        if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
                      "cudaFuncSetAttribute(k_convolve)")) { st = ARKCOS_ECUDA; break; }
-        if ((flags & ARKCOS_PLAN_PAIR_ROWS) &&
-            !cuda_ok(cudaFuncSetAttribute(k_convolve_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                     "cudaFuncSetAttribute(k_convolve_pairs)")) { st = ARKCOS_ECUDA; break; }
         size_t tab_bytes = (size_t)n_table * sizeof(double);
-        pl->table_in_smem = tab_bytes <= 200 * 1024 ? 1 : 0;
+        pl->table_in_smem = tab_bytes <= (size_t)kGenSmemMax ? 1 : 0;
         pl->gen_smem = pl->table_in_smem ? tab_bytes : 0;
-        if (!cuda_ok(cudaFuncSetAttribute(k_generate_weights, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(pl->gen_smem > 0 ? pl->gen_smem : 1)),
+        if (!cuda_ok(cudaFuncSetAttribute(k_generate_weights, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenSmemMax),
                      "cudaFuncSetAttribute(k_generate_weights)")) { st = ARKCOS_ECUDA; break; }
         const int units = (int)s.gen_units.size(), per_cta = kGenThreads / 32;
         const int want = (units + per_cta - 1) / per_cta;
         pl->gen_grid = want < pl->sm_count ? (want > 0 ? want : 1) : pl->sm_count;
-        for (auto& e : pl->ev)
-            if (!cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) { st = ARKCOS_ECUDA; break; }
-        if (st != ARKCOS_OK) break;
         if (flags & ARKCOS_PLAN_CACHE_WEIGHTS) {
             if ((st = launch_generate(pl, 0)) != ARKCOS_OK) break;
             if (!cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) { st = ARKCOS_ECUDA; break; }
@@ -252,42 +246,64 @@ arkcos_status arkcos_convolve(const arkcos_plan* pl, const float* d_in, float* d
     return arkcos_convolve_batch(pl, d_in, d_out, 1, stream);
 }
 
-arkcos_status arkcos_convolve_timed(const arkcos_plan* pl, const float* d_in, float* d_out, void* stream,
-                                    float* ms_generate, float* ms_convolve) {
-    arkcos_status s = check_io(pl, d_in, d_out, 1);
+arkcos_status arkcos_measure_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, void* stream,
+                                      float* ms_generate, float* ms_convolve) {
+    arkcos_status s = check_io(pl, d_in, d_out, n_maps);
     if (s != ARKCOS_OK) return s;
+    if (n_maps > 65535) return ARKCOS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const bool cached = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) != 0;
-    CU(cudaEventRecord(pl->ev[0], st));
-    if (!cached) { if ((s = launch_generate(pl, st)) != ARKCOS_OK) return s; }
-    CU(cudaEventRecord(pl->ev[1], st));
-    if ((s = launch_convolve(pl, d_in, d_out, 1, st)) != ARKCOS_OK) return s;
-    CU(cudaEventRecord(pl->ev[2], st));
-    CU(cudaEventSynchronize(pl->ev[2]));
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};             // per call: the entry point is re-entrant
+    for (auto& e : ev)
+        if (!cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) { for (auto& x : ev) if (x) cudaEventDestroy(x); return ARKCOS_ECUDA; }
     float a = 0.f, b = 0.f;
-    CU(cudaEventElapsedTime(&a, pl->ev[0], pl->ev[1]));
-    CU(cudaEventElapsedTime(&b, pl->ev[1], pl->ev[2]));
+    s = ARKCOS_ECUDA;
+    do {
+        if (!cuda_ok(cudaEventRecord(ev[0], st), "cudaEventRecord")) break;
+        if (!cached && (s = launch_generate(pl, st)) != ARKCOS_OK) break;
+        s = ARKCOS_ECUDA;
+        if (!cuda_ok(cudaEventRecord(ev[1], st), "cudaEventRecord")) break;
+        if ((s = launch_convolve(pl, d_in, d_out, n_maps, st)) != ARKCOS_OK) break;
+        s = ARKCOS_ECUDA;
+        if (!cuda_ok(cudaEventRecord(ev[2], st), "cudaEventRecord")) break;
+        if (!cuda_ok(cudaEventSynchronize(ev[2]), "cudaEventSynchronize")) break;
+        if (!cuda_ok(cudaEventElapsedTime(&a, ev[0], ev[1]), "cudaEventElapsedTime")) break;
+        if (!cuda_ok(cudaEventElapsedTime(&b, ev[1], ev[2]), "cudaEventElapsedTime")) break;
+        s = ARKCOS_OK;
+    } while (0);
+    for (auto& e : ev) cudaEventDestroy(e);
+    if (s != ARKCOS_OK) return s;
     if (ms_generate) *ms_generate = cached ? 0.f : a;
     if (ms_convolve) *ms_convolve = b;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_reserve_host_io(arkcos_plan* pl) {
+    if (!pl) return ARKCOS_EINVAL;
+    if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    if (pl->d_io_in) return ARKCOS_OK;
+    const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
+    cudaError_t e = cudaMalloc((void**)&pl->d_io_in, bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d_io_out, bytes);
+    if (e != cudaSuccess) {
+        cudaFree(pl->d_io_in); pl->d_io_in = nullptr; pl->d_io_out = nullptr;
+        if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); return ARKCOS_ENOMEM; }
+        CU(e);
+    }
+    pl->device_bytes += 2 * bytes;
     return ARKCOS_OK;
 }
 
 arkcos_status arkcos_convolve_host(arkcos_plan* pl, const float* h_in, float* h_out, void* stream) {
     if (!pl || !h_in || !h_out) return ARKCOS_EINVAL;
     if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
+    arkcos_status s = arkcos_plan_reserve_host_io(pl);           // no-op once reserved
+    if (s != ARKCOS_OK) return s;
+    if ((s = check_io(pl, pl->d_io_in, pl->d_io_out, 1)) != ARKCOS_OK) return s;
     const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
-    if (!pl->d_io_in) {
-        cudaError_t e = cudaMalloc((void**)&pl->d_io_in, bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d_io_out, bytes);
-        if (e == cudaErrorMemoryAllocation) {
-            (void)cudaGetLastError(); cudaFree(pl->d_io_in); pl->d_io_in = nullptr; return ARKCOS_ENOMEM;
-        }
-        CU(e);
-        pl->device_bytes += 2 * bytes;
-    }
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaMemcpyAsync(pl->d_io_in, h_in, bytes, cudaMemcpyHostToDevice, st));
-    arkcos_status s = run(pl, pl->d_io_in, pl->d_io_out, 1, st);
+    s = run(pl, pl->d_io_in, pl->d_io_out, 1, st);
     if (s != ARKCOS_OK) return s;
     CU(cudaMemcpyAsync(h_out, pl->d_io_out, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
@@ -315,6 +331,22 @@ arkcos_status arkcos_plan_get_info(const arkcos_plan* pl, arkcos_plan_info* info
     info->sm_count = pl->sm_count; info->flags = pl->flags; info->device_bytes = pl->device_bytes;
     info->fma_slots_wide = s.fma_slots_wide; info->first_narrow_ring = s.first_narrow;
     return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_item(const arkcos_plan* pl, int index, int* fields) {
+    if (!pl || !fields || index < 0 || index >= (int)pl->sched.items.size()) return ARKCOS_EINVAL;
+    const Item& it = pl->sched.items[index];
+    fields[0] = it.kind; fields[1] = it.i0; fields[2] = it.nrings; fields[3] = it.k0; fields[4] = kWarpSpan << it.f_log2;
+    fields[5] = kWarps >> it.f_log2;
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_plan_validate(const arkcos_plan* pl, char* why, int cap) {
+    if (!pl || cap < 0 || (cap > 0 && !why)) return ARKCOS_EINVAL;
+    std::string msg;
+    const int rc = validate_schedule(pl->sched, &msg);
+    if (cap > 0) { std::strncpy(why, msg.c_str(), (size_t)cap - 1); why[cap - 1] = 0; }
+    return rc == 0 ? ARKCOS_OK : ARKCOS_EINTERNAL;
 }
 
 arkcos_status arkcos_plan_window(const arkcos_plan* pl, int i, int j, int* half_width) {

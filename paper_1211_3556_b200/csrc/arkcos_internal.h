@@ -2,6 +2,7 @@
 // Product code; shares nothing with oracle/.
 #pragma once
 #include <cstdint>
+#include <string>
 #include <vector>
 
 #ifdef __CUDACC__
@@ -64,16 +65,6 @@ struct NarrowRun {
     int32_t pad_;
 };
 
-// EXPERIMENTAL (ARKCOS_PLAN_PAIR_ROWS): a run of the paired-rows narrow path.  The two mirror input rows
-// i - q and i + q of a ring have (after taking the union) the same window, so one run slides two register
-// windows over the same taps: twice the FMAs per run start.  Entry e of a ring's list; n = 0 ends the list.
-struct PairRun {
-    int32_t wq_rel_a;   // byte offset of row a's weights in the ring's block, minus 8 * k0
-    int32_t wq_rel_b;   // ... of row b's (paired runs)
-    int32_t k0n;        // k0 | n << 8 | paired << 16
-    int32_t rows;       // row index (0 .. 2R) of a | of b << 8
-};
-
 enum ItemKind : int16_t { kWide = 0, kNarrow = 1 };
 
 // One CTA of the convolution launch.
@@ -113,8 +104,6 @@ struct Schedule {
     std::vector<double> s2;                 // [n_phi/2+1] sin^2(d dphi / 2)
     std::vector<PairDesc> pairs;            // [n_north][2R+1]
     std::vector<NarrowRun> runs;            // [n_north - first_narrow][2R+1]
-    std::vector<PairRun> pair_runs;         // [n_north - first_narrow][2R+1], only with pair_rows
-    bool pair_rows = false;                 // EXPERIMENTAL paired-rows narrow path
     uint32_t narrow_w_base = 0;             // weights of narrow ring i start at narrow_w_base + (i - first_narrow) * narrow_wslot
     std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
     std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows, padded to 4)
@@ -144,6 +133,14 @@ size_t wide_smem_bytes(int R);
 size_t narrow_smem_bytes(int f_log2, int R, int wslot);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out, bool pair_rows = false);
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);
+
+// Re-derives, as plain integer arithmetic, every global-memory range and every shared-memory offset the
+// kernels will form from the schedule's descriptors (work items, pair descriptors, narrow runs, generator
+// units) and checks that each lies inside its buffer, is aligned as the instruction that uses it needs, and
+// that every input ring a non-empty pair names exists.  Called by build_schedule before it returns (a
+// schedule that fails is never uploaded: arkcos_plan_create returns ARKCOS_EINTERNAL) and by the CPU tests on
+// every BASELINE.json workload.  Returns 0, or a positive code; `why` (may be null) receives a description.
+int validate_schedule(const Schedule& s, std::string* why);
 
 }  // namespace arkcos

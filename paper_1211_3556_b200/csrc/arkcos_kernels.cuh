@@ -33,6 +33,7 @@ struct GenParams {
 };
 
 constexpr int kGenThreads = 512;
+constexpr int kGenSmemMax = 200 * 1024;   // largest table (bytes) the generator keeps in shared memory
 
 __device__ __forceinline__ float gen_weight(const GenParams& p, const GenUnit& g, const double* tab, const int d) {
     const int ad = d < 0 ? -d : d;
@@ -102,7 +103,6 @@ struct ConvParams {
     const Item* items;
     const float* weights;
     const NarrowRun* runs;   // [n_north - first_narrow][2R+1]
-    const PairRun* pair_runs;   // same shape; EXPERIMENTAL paired-rows path only
     int n_theta, n_phi, R;
     int first_narrow;        // first northern ring of the narrow class
     uint32_t narrow_w_base;  // its weights start here; one block of wslot floats per narrow ring
@@ -424,53 +424,8 @@ nr_done:;
 }
 #pragma nv_diag_default 177
 
-// ---- EXPERIMENTAL paired-rows chain (ARKCOS_PLAN_PAIR_ROWS) ---------------------------------------------
-// The mirror input rows i-q and i+q of a ring share one window, so one run slides TWO register windows
-// over the same taps: a step is 128 FFMA for 4 LDS.64, and a ring has R+1 run starts instead of 2R+1.
-// Windows of paired runs lie inside [-16, 16): the chain has the 16 steps K = 8 .. 23.
-template <int K>
-__device__ __forceinline__ void pair_step(float (&a0)[kLaneP], float (&a1)[kLaneP], float (&za)[2 * kNarrowPairs],
-                                          float (&zb)[2 * kNarrowPairs], float (&wa)[2][2], float (&wb)[2][2],
-                                          const uint32_t zta, const uint32_t ztb, const uint32_t wqa, const uint32_t wqb) {
-    constexpr int N = 2 * ((K + 17) % kNarrowPairs);
-    lds64i<narrow_pair_off(K + 17)>(za[N], za[N + 1], zta);
-    lds64i<narrow_pair_off(K + 17)>(zb[N], zb[N + 1], ztb);
-    lds64i<8 * (K + 1)>(wa[(K + 1) & 1][0], wa[(K + 1) & 1][1], wqa);
-    lds64i<8 * (K + 1)>(wb[(K + 1) & 1][0], wb[(K + 1) & 1][1], wqb);
-#pragma unroll
-    for (int m = 0; m < kLaneP; m++) a0[m] = fmaf(za[(2 * K + m) % (2 * kNarrowPairs)], wa[K & 1][0], a0[m]);
-#pragma unroll
-    for (int m = 0; m < kLaneP; m++) a1[m] = fmaf(za[(2 * K + m + 1) % (2 * kNarrowPairs)], wa[K & 1][1], a1[m]);
-#pragma unroll
-    for (int m = 0; m < kLaneP; m++) a0[m] = fmaf(zb[(2 * K + m) % (2 * kNarrowPairs)], wb[K & 1][0], a0[m]);
-#pragma unroll
-    for (int m = 0; m < kLaneP; m++) a1[m] = fmaf(zb[(2 * K + m + 1) % (2 * kNarrowPairs)], wb[K & 1][1], a1[m]);
-}
-
-#pragma nv_diag_suppress 177
-__device__ __forceinline__ void narrow_pair_row(float (&a0)[kLaneP], float (&a1)[kLaneP], const uint32_t zta, const uint32_t ztb,
-                                                const uint32_t wqa, const uint32_t wqb, const int k0, int n) {
-    float za[2 * kNarrowPairs], zb[2 * kNarrowPairs];
-    float wa[2][2], wb[2][2];
-#define ARKCOS_PR_CASE(K) case K: narrow_init<K>(za, wa, zta, wqa); narrow_init<K>(zb, wb, ztb, wqb); goto pr_step_##K;
-#define ARKCOS_PR_STEP(K) pr_step_##K: pair_step<K>(a0, a1, za, zb, wa, wb, zta, ztb, wqa, wqb); if (--n == 0) goto pr_done;
-    switch (k0) {
-        ARKCOS_PR_CASE(8) ARKCOS_PR_CASE(9) ARKCOS_PR_CASE(10) ARKCOS_PR_CASE(11) ARKCOS_PR_CASE(12) ARKCOS_PR_CASE(13)
-        ARKCOS_PR_CASE(14) ARKCOS_PR_CASE(15) ARKCOS_PR_CASE(16)
-        default: return;
-    }
-    ARKCOS_PR_STEP(8) ARKCOS_PR_STEP(9) ARKCOS_PR_STEP(10) ARKCOS_PR_STEP(11) ARKCOS_PR_STEP(12) ARKCOS_PR_STEP(13)
-    ARKCOS_PR_STEP(14) ARKCOS_PR_STEP(15) ARKCOS_PR_STEP(16) ARKCOS_PR_STEP(17) ARKCOS_PR_STEP(18) ARKCOS_PR_STEP(19)
-    ARKCOS_PR_STEP(20) ARKCOS_PR_STEP(21) ARKCOS_PR_STEP(22) ARKCOS_PR_STEP(23)
-pr_done:;
-#undef ARKCOS_PR_CASE
-#undef ARKCOS_PR_STEP
-}
-#pragma nv_diag_default 177
-
 // A band of `nr` rings of one hemisphere, in "logical" (northern) ring indices lam: the physical ring of
 // logical ring lam is lam (north) or n_theta-1-lam (south); descriptors and weights are those of lam.
-template <bool PAIRS>
 __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, const float* in, float* out) {
     const int F = 1 << it.f_log2, S = kWarps >> it.f_log2;
     const bool south = it.nrings < 0;
@@ -513,7 +468,7 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
         for (int rs = 0; rs < S; rs++) {
             const int lam = lam0 + pass * S + rs;
             if (lam >= lam_end) break;
-            const NarrowRun* psrc = (PAIRS ? reinterpret_cast<const NarrowRun*>(p.pair_runs) : p.runs) + (size_t)(lam - p.first_narrow) * W;
+            const NarrowRun* psrc = p.runs + (size_t)(lam - p.first_narrow) * W;
             const uint32_t pdst = pdbuf_addr + (uint32_t)(((b * S + rs) * W) * sizeof(NarrowRun));
             for (int q = threadIdx.x; q < W; q += kThreads) cp_async16(pdst + 16 * q, psrc + q);
             const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
@@ -544,44 +499,19 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
             int slot = (lam - p.R) % NS; if (slot < 0) slot += NS;
             uint32_t zt = rows + (uint32_t)(slot * slot_bytes) + lane_tile;
             const uint32_t zt_end = rows + (uint32_t)(NS * slot_bytes) + lane_tile;
-            if constexpr (!PAIRS) {
-                // Run descriptors are double buffered in registers: the descriptor of run r+1 is loaded into
-                // the other set while run r executes, and only copied out of it one run later.
-                int dA[4], dB[4];
-                lds128u(dA[0], dA[1], dA[2], dA[3], spd);
-    #pragma unroll 1
-                for (int r = 0; r < W; r++) {
-                    const uint32_t nxt = spd + (uint32_t)((r + 1 < W ? r + 1 : r) * sizeof(NarrowRun));
-                    int wq_rel, k0, n;
-                    if (r & 1) { wq_rel = dB[0]; k0 = dB[1]; n = dB[2]; lds128u(dA[0], dA[1], dA[2], dA[3], nxt); }
-                    else { wq_rel = dA[0]; k0 = dA[1]; n = dA[2]; lds128u(dB[0], dB[1], dB[2], dB[3], nxt); }
-                    if (n != 0) narrow_row(a0, a1, zt, wring + (uint32_t)wq_rel, k0, n);
-                    zt += (uint32_t)slot_bytes;
-                    if (zt == zt_end) zt -= (uint32_t)(NS * slot_bytes);
-                }
-            } else {
-                // EXPERIMENTAL: run list of PairRun entries (n = 0 ends it), rows addressed by index
-                int slot0 = (lam - p.R) % NS; if (slot0 < 0) slot0 += NS;
-                int dA[4], dB[4];
-                lds128u(dA[0], dA[1], dA[2], dA[3], spd);
+            // Run descriptors are double buffered in registers: the descriptor of run r+1 is loaded into
+            // the other set while run r executes, and only copied out of it one run later.
+            int dA[4], dB[4];
+            lds128u(dA[0], dA[1], dA[2], dA[3], spd);
 #pragma unroll 1
-                for (int e = 0; e < W; e++) {
-                    const uint32_t nxt = spd + (uint32_t)((e + 1 < W ? e + 1 : e) * sizeof(PairRun));
-                    int wqa, wqb, k0n, rr;
-                    if (e & 1) { wqa = dB[0]; wqb = dB[1]; k0n = dB[2]; rr = dB[3]; lds128u(dA[0], dA[1], dA[2], dA[3], nxt); }
-                    else { wqa = dA[0]; wqb = dA[1]; k0n = dA[2]; rr = dA[3]; lds128u(dB[0], dB[1], dB[2], dB[3], nxt); }
-                    const int k0 = k0n & 0xff, n = (k0n >> 8) & 0xff;
-                    if (n == 0) break;
-                    int sa = slot0 + (rr & 0xff); if (sa >= NS) sa -= NS;
-                    const uint32_t zta = rows + (uint32_t)(sa * slot_bytes) + lane_tile;
-                    if (k0n >> 16) {
-                        int sb = slot0 + (rr >> 8); if (sb >= NS) sb -= NS;
-                        narrow_pair_row(a0, a1, zta, rows + (uint32_t)(sb * slot_bytes) + lane_tile, wring + (uint32_t)wqa,
-                                        wring + (uint32_t)wqb, k0, n);
-                    } else {
-                        narrow_row(a0, a1, zta, wring + (uint32_t)wqa, k0, n);
-                    }
-                }
+            for (int r = 0; r < W; r++) {
+                const uint32_t nxt = spd + (uint32_t)((r + 1 < W ? r + 1 : r) * sizeof(NarrowRun));
+                int wq_rel, k0, n;
+                if (r & 1) { wq_rel = dB[0]; k0 = dB[1]; n = dB[2]; lds128u(dA[0], dA[1], dA[2], dA[3], nxt); }
+                else { wq_rel = dA[0]; k0 = dA[1]; n = dA[2]; lds128u(dB[0], dB[1], dB[2], dB[3], nxt); }
+                if (n != 0) narrow_row(a0, a1, zt, wring + (uint32_t)wq_rel, k0, n);
+                zt += (uint32_t)slot_bytes;
+                if (zt == zt_end) zt -= (uint32_t)(NS * slot_bytes);
             }
             const int phi = it.k0 + f * kWarpSpan + lane * kLaneP;
             float* orow = out + (size_t)(south ? p.n_theta - 1 - lam : lam) * p.n_phi + phi;
@@ -602,26 +532,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_convolve(const ConvParams p) {
     char* smem = reinterpret_cast<char*>(emu::g_smem);
 #endif
     const Item it = p.items[blockIdx.x];
+    // The descriptors were validated on the host (validate_schedule) before they were uploaded; this guard only
+    // keeps a work item that was corrupted in device memory from being turned into addresses.
+    if ((unsigned)it.f_log2 > 3u || (unsigned)it.k0 >= (unsigned)p.n_phi || (unsigned)it.i0 >= (unsigned)p.n_theta ||
+        (it.kind != kWide && it.kind != kNarrow)) return;
     const float* in = p.in + (long long)blockIdx.y * p.map_stride;
     float* out = p.out + (long long)blockIdx.y * p.map_stride;
     if (it.kind == kWide) conv_wide(p, it, smem, in, out);
-    else conv_narrow<false>(p, it, smem, in, out);
-}
-
-// EXPERIMENTAL (ARKCOS_PLAN_PAIR_ROWS): same launch, paired-rows narrow path.  A separate kernel so that the
-// default kernel's code is untouched until this one has been measured.
-__global__ void __launch_bounds__(kThreads, 1) k_convolve_pairs(const ConvParams p) {
-#ifndef ARKCOS_HOST_EMU
-    extern __shared__ uint4 smem4[];
-    char* smem = reinterpret_cast<char*>(smem4);
-#else
-    char* smem = reinterpret_cast<char*>(emu::g_smem);
-#endif
-    const Item it = p.items[blockIdx.x];
-    const float* in = p.in + (long long)blockIdx.y * p.map_stride;
-    float* out = p.out + (long long)blockIdx.y * p.map_stride;
-    if (it.kind == kWide) conv_wide(p, it, smem, in, out);
-    else conv_narrow<true>(p, it, smem, in, out);
+    else conv_narrow(p, it, smem, in, out);
 }
 
 }  // namespace arkcos

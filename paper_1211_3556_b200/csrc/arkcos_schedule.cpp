@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <string>
 
 #include "arkcos_internal.h"
 
@@ -45,13 +46,12 @@ int Schedule::window(int i, int j) const {
     return window_of(*this, i, j);
 }
 
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s, bool pair_rows) {
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s) {
     if (n_theta < 1 || n_phi < 4 || !(theta_cut > 0.0) || !(theta_cut <= kPi * (1.0 + 1e-15))) return 1;
     if (n_phi % 4 != 0) return 4;
     if (sm_count < 1) sm_count = 148;
     s = Schedule();
     s.n_theta = n_theta; s.n_phi = n_phi; s.theta_cut = theta_cut;
-    s.pair_rows = pair_rows;
     s.n_north = (n_theta + 1) / 2;
     const double dtheta = kPi / n_theta, dphi = 2.0 * kPi / n_phi;
     {
@@ -119,26 +119,13 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     };
     s.first_narrow = s.n_north;
     while (s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
-    // stored windows of the narrow rings.  Paired-rows path: the mirror rows i-q, i+q of a ring get the union
-    // of their two windows when it fits [-16, 16) (they differ by a tap at most: D ~ 1/sqrt(sin t_i sin t_j)).
+    // stored windows of the narrow rings
     std::vector<int> nw_start((size_t)s.n_north * W, 0), nw_ntaps((size_t)s.n_north * W, 0);
-    std::vector<char> nw_paired((size_t)s.n_north * W, 0);
-    for (int i = s.first_narrow; i < s.n_north; i++) {
+    for (int i = s.first_narrow; i < s.n_north; i++)
         for (int r = 0; r < W; r++) {
             const PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half >= 0) narrow_range(p.half, nw_start[(size_t)i * W + r], nw_ntaps[(size_t)i * W + r]);
         }
-        if (!pair_rows) continue;
-        for (int q = 1; q <= s.R; q++) {
-            const size_t a = (size_t)i * W + (s.R - q), b = (size_t)i * W + (s.R + q);
-            if (s.pairs[a].half < 0 || s.pairs[b].half < 0) continue;
-            const int st = std::min(nw_start[a], nw_start[b]);
-            const int en = std::max(nw_start[a] + nw_ntaps[a], nw_start[b] + nw_ntaps[b]);
-            if (st < -16 || en > 16) continue;
-            nw_start[a] = nw_start[b] = st; nw_ntaps[a] = nw_ntaps[b] = en - st;
-            nw_paired[a] = nw_paired[b] = 1;
-        }
-    }
     {
         unsigned long long wslot = 0;
         for (int i = s.first_narrow; i < s.n_north; i++) {
@@ -150,7 +137,6 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     }
     int nf_cap = 0;                                           // largest useful F of the narrow tiles
     while (nf_cap < 3 && (kWarpSpan << nf_cap) < n_phi) nf_cap++;
-    if (const char* e = std::getenv("ARKCOS_NARROW_F_LOG2")) nf_cap = std::min(nf_cap, std::max(0, std::atoi(e)));   // tuning knob
     s.narrow_f_log2 = -1;
     for (int fl = nf_cap; fl >= 0; fl--)
         if (narrow_smem_bytes(fl, s.R, s.narrow_wslot) <= (size_t)kSmemBudget) { s.narrow_f_log2 = fl; break; }
@@ -194,23 +180,6 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             u.n = p.ntaps / 2;
             u.wq_rel = 4 * (int32_t)(p.w_off - s.ring_w_off[i]) - 8 * u.k0;
         }
-    if (pair_rows) {
-        s.pair_runs.assign((size_t)(s.n_north - s.first_narrow) * W, PairRun{0, 0, 0, 0});
-        for (int i = s.first_narrow; i < s.n_north; i++) {
-            PairRun* list = &s.pair_runs[(size_t)(i - s.first_narrow) * W];
-            int e = 0;
-            auto rel = [&](int r, int k0) { return 4 * (int32_t)(s.pairs[(size_t)i * W + r].w_off - s.ring_w_off[i]) - 8 * k0; };
-            for (int r = 0; r < W; r++) {
-                const PairDesc& p = s.pairs[(size_t)i * W + r];
-                if (p.ntaps == 0) continue;
-                const bool paired = nw_paired[(size_t)i * W + r] != 0;
-                if (paired && r > s.R) continue;                        // emitted with its mirror row
-                const int k0 = (kHaloNarrow + p.start) / 2, n = p.ntaps / 2;
-                const int rb = paired ? 2 * s.R - r : r;
-                list[e++] = PairRun{rel(r, k0), rel(rb, k0), k0 | (n << 8) | ((paired ? 1 : 0) << 16), r | (rb << 8)};
-            }
-        }
-    }
 
     // ---- generator work units: one warp writes up to kGenUnitTaps taps (steps) of one ring pair -----
     for (int i = 0; i < s.n_north; i++) {
@@ -288,6 +257,117 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
     s.items.reserve(tmp.size());
     for (auto& t : tmp) s.items.push_back(t.it);
+    return validate_schedule(s, nullptr) == 0 ? 0 : 5;
+}
+
+// ---- validate_schedule ---------------------------------------------------------------------------
+// Every check below restates, in integers, an address the kernels of arkcos_kernels.cuh form from the
+// descriptor it names (the function and line of thought are given with each group).  The kernels trust the
+// descriptors: there is no bounds check in the hot loops, so nothing that fails here may reach the device.
+int validate_schedule(const Schedule& s, std::string* why) {
+    int code = 0;
+    auto fail = [&](int c, const char* what, long long a, long long b) {
+        if (code == 0) {
+            code = c;
+            if (why) *why = std::string(what) + " (" + std::to_string(a) + ", " + std::to_string(b) + ")";
+        }
+        return c;
+    };
+    const int W = 2 * s.R + 1, n_theta = s.n_theta, n_phi = s.n_phi;
+    if (n_theta < 1 || n_phi < 4 || n_phi % 4 != 0 || s.R < 0 || s.R >= n_theta) return fail(1, "grid / R", n_phi, s.R);
+    if (s.n_north != (n_theta + 1) / 2 || s.first_narrow < 0 || s.first_narrow > s.n_north) return fail(2, "ring classes", s.first_narrow, s.n_north);
+    if (s.pairs.size() != (size_t)s.n_north * W) return fail(3, "pairs size", (long long)s.pairs.size(), W);
+    if (s.runs.size() != (size_t)(s.n_north - s.first_narrow) * W) return fail(4, "runs size", (long long)s.runs.size(), W);
+    if (s.s2.size() != (size_t)n_phi / 2 + 1) return fail(5, "s2 size", (long long)s.s2.size(), n_phi);
+    if (s.ring_w_off.size() != (size_t)s.n_north || s.ring_slots.size() != (size_t)s.n_north) return fail(6, "ring tables", 0, 0);
+    if (s.weight_slots > 0xFFFFFFF0ull) return fail(7, "weight buffer over 2^32 floats", (long long)s.weight_slots, 0);
+    if (s.smem_bytes > (size_t)kSmemBudget) return fail(8, "shared memory over budget", (long long)s.smem_bytes, kSmemBudget);
+    const long long wtot = (long long)s.weight_slots;
+    const bool have_narrow = s.first_narrow < s.n_north;
+    if (have_narrow) {
+        if (s.narrow_f_log2 < 0 || s.narrow_f_log2 > 3) return fail(9, "narrow_f_log2", s.narrow_f_log2, 0);
+        if (s.narrow_wslot < 4 || s.narrow_wslot % 4 != 0 || s.narrow_w_base % 4 != 0) return fail(10, "narrow weight stride", s.narrow_wslot, s.narrow_w_base);
+        if (narrow_smem_bytes(s.narrow_f_log2, s.R, s.narrow_wslot) > s.smem_bytes) return fail(11, "narrow shared memory", 0, 0);
+    }
+    if (s.first_narrow > 0 && wide_smem_bytes(s.R) > s.smem_bytes) return fail(12, "wide shared memory", 0, 0);
+
+    // ---- pair descriptors (conv_wide: stage source rows and weight ranges; plan_pair_weights) ----------
+    unsigned long long stored = 0;
+    for (int i = 0; i < s.n_north; i++) {
+        const bool wide = i < s.first_narrow;
+        unsigned long long ring = 0;
+        for (int r = 0; r < W; r++) {
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            const int j = i + r - s.R;
+            if (p.ntaps == 0) { if (p.half >= 0) return fail(20, "in-support pair without stored taps", i, r); continue; }
+            if (p.half < 0 || j < 0 || j >= n_theta) return fail(21, "stored taps for a ring pair that does not exist", i, j);
+            const int q = wide ? 4 : 2;                          // conv_wide: 16-byte steps; conv_narrow: 8-byte steps
+            if (p.ntaps < 0 || p.ntaps % q || p.start > 0 || (-p.start) % q || p.w_off % q) return fail(22, "tap range granularity", i, r);
+            if (p.half != n_phi && (p.half >= n_phi / 2 || p.start > -p.half || p.start + p.ntaps <= p.half)) return fail(23, "stored range does not cover the window", i, r);
+            if (p.half == n_phi && (p.start > -(n_phi / 2) || p.start + p.ntaps < n_phi / 2)) return fail(24, "stored range does not cover the whole ring", i, r);
+            if (-p.start > n_phi / 2 + 3 || p.start + p.ntaps > n_phi / 2 + 4) return fail(25, "stored range beyond one turn", i, r);
+            if ((long long)p.w_off + p.ntaps > wtot) return fail(26, "weights beyond the buffer", i, r);
+            if ((long long)p.w_off < s.ring_w_off[i] || (long long)p.w_off + p.ntaps > (long long)s.ring_w_off[i] + s.ring_slots[i]) return fail(27, "weights outside the ring's block", i, r);
+            if (!wide && (p.start < -kHaloNarrow || p.start + p.ntaps > kHaloNarrow)) return fail(28, "narrow window outside the halo", i, r);
+            ring += (unsigned long long)p.ntaps;
+        }
+        if (((ring + 3) & ~3ull) != s.ring_slots[i]) return fail(29, "ring_slots", i, (long long)ring);
+        if (!wide && (s.ring_w_off[i] != s.narrow_w_base + (unsigned long long)(i - s.first_narrow) * s.narrow_wslot ||
+                      s.ring_slots[i] > (unsigned)s.narrow_wslot)) return fail(30, "narrow ring block", i, s.ring_slots[i]);
+        stored += ring;
+    }
+    // ---- narrow run descriptors (conv_narrow / narrow_row: jump-table entry, step count, weight address) ---
+    for (int i = s.first_narrow; i < s.n_north; i++)
+        for (int r = 0; r < W; r++) {
+            const NarrowRun& u = s.runs[(size_t)(i - s.first_narrow) * W + r];
+            const PairDesc& p = s.pairs[(size_t)i * W + r];
+            if (u.n == 0) { if (p.ntaps != 0) return fail(40, "pair without a run", i, r); continue; }
+            if (u.k0 < 0 || u.k0 > 16 || u.n < 1 || u.k0 + u.n > kHaloNarrow) return fail(41, "run outside the step chain", u.k0, u.n);
+            if (2 * u.k0 - kHaloNarrow != p.start || 2 * u.n != p.ntaps) return fail(42, "run does not match its pair", i, r);
+            const long long woff = (long long)u.wq_rel + 8ll * u.k0;       // byte offset of the run's weights in the ring block
+            if (woff < 0 || woff % 8 || woff != 4ll * (p.w_off - s.ring_w_off[i])) return fail(43, "run weight offset", i, r);
+            if (woff / 4 + p.ntaps > (long long)s.ring_slots[i]) return fail(44, "run weights beyond the staged block", i, r);
+        }
+    // ---- generator units (k_generate_weights: destination range, s2 index) ---------------------------------
+    unsigned long long gen = 0;
+    for (const GenUnit& g : s.gen_units) {
+        if (g.count < 1 || g.count > kGenUnitTaps || (long long)g.w_base + g.count > wtot) return fail(50, "generator unit range", g.w_base, g.count);
+        if (!(g.half == n_phi || (g.half >= 0 && g.half < n_phi / 2))) return fail(51, "generator unit window", g.half, 0);
+        const long long lo = g.d0, hi = (long long)g.d0 + g.count - 1;   // taps written; inside-the-window taps index s2[|d|]
+        if (lo < -(long long)(n_phi / 2) - 3 || hi > n_phi / 2 + 3) return fail(52, "generator unit taps beyond one turn", lo, hi);
+        gen += (unsigned long long)g.count;
+    }
+    if (gen != stored) return fail(53, "generator units do not tile the stored taps", (long long)gen, (long long)stored);
+    // ---- work items (k_convolve) and coverage: every output ring x warp tile exactly once -----------------
+    const int tiles = (n_phi + kWarpSpan - 1) / kWarpSpan;
+    std::vector<unsigned char> cover((size_t)n_theta * tiles, 0);
+    for (const Item& it : s.items) {
+        if (it.f_log2 < 0 || it.f_log2 > 3) return fail(60, "item f_log2", it.f_log2, 0);
+        const int L = kWarpSpan << it.f_log2;
+        if (it.k0 < 0 || it.k0 >= n_phi || it.k0 % L) return fail(61, "item k0", it.k0, L);
+        const int t0 = it.k0 / kWarpSpan, t1 = std::min(tiles, t0 + (1 << it.f_log2));
+        if (it.kind == kWide) {
+            if (it.i0 < 0 || it.i0 >= n_theta) return fail(62, "wide item ring", it.i0, 0);
+            const int i_n = 2 * it.i0 >= n_theta ? n_theta - 1 - it.i0 : it.i0;
+            if (i_n >= s.first_narrow) return fail(63, "wide item on a narrow ring", it.i0, s.first_narrow);
+            for (int t = t0; t < t1; t++) cover[(size_t)it.i0 * tiles + t]++;
+        } else if (it.kind == kNarrow) {
+            const int nr = it.nrings < 0 ? -it.nrings : it.nrings;
+            if (!have_narrow || it.f_log2 != s.narrow_f_log2) return fail(64, "narrow item tile", it.f_log2, s.narrow_f_log2);
+            if (nr < 1 || it.i0 < s.first_narrow || it.i0 + nr > s.n_north) return fail(65, "narrow item band", it.i0, nr);
+            if (it.wcopy < 4 || it.wcopy % 4 || it.wcopy > s.narrow_wslot) return fail(66, "narrow item wcopy", it.wcopy, s.narrow_wslot);
+            // stage_ring_tables reads wcopy floats of each ring's block
+            if ((long long)s.narrow_w_base + (long long)(it.i0 + nr - 1 - s.first_narrow) * s.narrow_wslot + it.wcopy > wtot) return fail(67, "narrow weight block beyond the buffer", it.i0, nr);
+            for (int q = 0; q < nr; q++) {
+                if (s.ring_slots[it.i0 + q] > (unsigned)it.wcopy) return fail(68, "ring block larger than wcopy", it.i0 + q, it.wcopy);
+                const int i_phys = it.nrings < 0 ? n_theta - 1 - (it.i0 + q) : it.i0 + q;
+                if (it.nrings < 0 && 2 * (it.i0 + q) + 1 == n_theta) return fail(69, "self-mirrored ring in a southern band", it.i0 + q, 0);
+                for (int t = t0; t < t1; t++) cover[(size_t)i_phys * tiles + t]++;
+            }
+        } else return fail(70, "item kind", it.kind, 0);
+    }
+    for (size_t c = 0; c < cover.size(); c++)
+        if (cover[c] != 1) return fail(71, "output tile not written exactly once (ring, count)", (long long)(c / tiles), cover[c]);
     return 0;
 }
 

@@ -210,6 +210,17 @@ def by_name(name: str) -> Workload:
     raise KeyError(name)
 
 
+def paper_regime_workload(theta_cut_arcmin: float = 240.0) -> Workload:
+    """SURVEY §8(f) N3, second half: the paper's own radius.  PAPER.md:L104 (§3) works its example at
+    theta_cut = 240 arcmin on nside 2048 (here: the 4096 x 8192 ECP grid that stands in for it, R = 91), with
+    an oscillatory real-space split kernel; the residual kernel of configs[4] (Gaussian FWHM 10' minus its
+    l <= 600 part) is the synthetic stand-in for the paper's fitted kernel (unspecified).
+    Tabulated by the caller on the paper's two-zone nodes: see `biased_nodes`."""
+    return Workload(f"paper_4096x8192_resid10_cut{theta_cut_arcmin:g}", 4096, 8192, theta_cut_arcmin * ARCMIN, 16384,
+                    "residual", _g(10.0), (20,), l_band=600,
+                    note="the paper's regime (PAPER.md:L104): theta_cut 240', oscillatory kernel; not a BASELINE config")
+
+
 def small_selfcheck_workload() -> Workload:
     """SURVEY §8(c) 'recommended extra self-check configuration': 128x256, Gaussian FWHM 240',
     cut = 3 FWHM - the px-per-sigma ratios of configs[2], O(N^2) feasible."""

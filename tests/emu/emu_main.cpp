@@ -124,8 +124,7 @@ int main(int argc, char** argv) {
     std::vector<float> out(n_pix, std::nanf(""));
 
     Schedule s;
-    const bool pair_rows = std::getenv("EMU_PAIR_ROWS") != nullptr;        // experimental paired-rows narrow path
-    const int rc = build_schedule(n_theta, n_phi, theta_cut, 148, s, pair_rows);
+    const int rc = build_schedule(n_theta, n_phi, theta_cut, 148, s);
     if (rc != 0) { std::fprintf(stderr, "build_schedule failed: %d\n", rc); return 2; }
     if (s.smem_bytes > (size_t)kSmemBudget) { std::fprintf(stderr, "shared memory over budget\n"); return 2; }
     std::vector<float> weights((size_t)s.weight_slots + 4, 0.0f);
@@ -152,11 +151,10 @@ int main(int argc, char** argv) {
     // ---- S3: convolution, one CTA per work item ------------------------------------------------------
     ConvParams c;
     c.in = in.data(); c.out = out.data(); c.pairs = s.pairs.data(); c.items = s.items.data(); c.weights = weights.data();
-    c.runs = s.runs.data(); c.pair_runs = s.pair_runs.data(); c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
+    c.runs = s.runs.data(); c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
     c.n_theta = n_theta; c.n_phi = n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
     c.map_stride = (long long)n_pix;
     emu::g_global.push_back({(const unsigned char*)s.runs.data(), (const unsigned char*)(s.runs.data() + s.runs.size())});
-    emu::g_global.push_back({(const unsigned char*)s.pair_runs.data(), (const unsigned char*)(s.pair_runs.data() + s.pair_runs.size())});
     emu::g_gridDim = dim3((unsigned)s.items.size());
     int n_wide = 0, n_narrow = 0;
     // EMU_ITEM_STRIDE=n: run every n-th work item only (big grids; outputs of the skipped items stay NaN)
@@ -166,14 +164,11 @@ int main(int argc, char** argv) {
         if (item_stride > 1 && b % item_stride != 0) continue;
         if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
         (wide ? n_wide : n_narrow)++;
-        emu::run_cta((unsigned)b, 0, kThreads, s.smem_bytes, [&] { if (pair_rows) k_convolve_pairs(c); else k_convolve(c); });
+        emu::run_cta((unsigned)b, 0, kThreads, s.smem_bytes, [&] { k_convolve(c); });
     }
     FILE* f = std::fopen(argv[7], "wb");
     if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
     std::fclose(f);
-    int n_paired = 0;
-    for (const auto& u : s.pair_runs) n_paired += (u.k0n >> 16) & 1;
-    std::printf("paired runs %d; ", n_paired);
     std::printf("emu ok: R %d first_narrow %d n_north %d narrow_f_log2 %d items wide %d narrow %d smem %zu weight_slots %llu\n", s.R,
                 s.first_narrow, s.n_north, s.narrow_f_log2, n_wide, n_narrow, s.smem_bytes, (unsigned long long)s.weight_slots);
     return 0;

@@ -148,7 +148,7 @@ def test_cached_batch_host_and_repeat_calls_are_bit_identical(torch, arkcos):
         h_out = np.empty_like(maps[0])
         plan.convolve_host(maps[0], h_out, stream)
         assert (h_out == single[0].cpu().numpy()).all()
-        gen_ms, conv_ms = plan.convolve_timed(d_in[0], again[0], stream)
+        gen_ms, conv_ms = plan.measure_convolve(d_in[0], again[0], stream)
         assert gen_ms > 0 and conv_ms > 0 and torch.equal(again[0], single[0])
 
 
@@ -183,40 +183,90 @@ def test_config1_full_map_and_golden(torch, arkcos):
 
 
 # ------------------------------------------------------------------ full-size configs: sampled ---
-def sample_pixels(w, n_random, seed, plan_r):
-    """All tile seams, pole rings, the equator and seeded random pixels (SURVEY §8(c)-6 subset idea)."""
+ORACLE_PAIR_BUDGET = 4.0e9      # in-support pairs the oracle evaluates per workload (~10 s on the GPU box's 16 cores)
+
+
+def seam_ks(nph, rng):
+    """phi positions at every seam of the kernels' tiling: the lane tile (32), the warp tile (1024) and
+    the CTA tile (multiples of 1024 up to 8192), the wrap-around at 0 / n_phi, plus seeded random ones."""
+    ks = {0, 1, 2, 3, 4, 15, 16, 17, 31, 32, 33, 63, 64, 511, 512, 513, nph // 2 - 1, nph // 2, nph - 33, nph - 32, nph - 17, nph - 1}
+    for m in range(1, nph // 1024 + 1):
+        ks |= {m * 1024 - 1, m * 1024, m * 1024 + 1}
+    ks |= {int(k) for k in rng.integers(0, nph, size=12)}
+    return sorted(k for k in ks if 0 <= k < nph)
+
+
+def ring_taps(plan, i, nt, nph, r):
+    t = 0
+    for j in range(max(0, i - r), min(nt, i + r + 1)):
+        d = plan.window(i, j)
+        t += nph if d == nph else (2 * d + 1 if d >= 0 else 0)
+    return t
+
+
+def probe_pixels(w, plan, seed):
+    """Pixels the oracle evaluates for a full-size workload: WHOLE rings (all k) at the seams of the schedule -
+    the WIDE/NARROW class boundary, a boundary between two NARROW bands, the equator, and as many of the polar
+    rings 0 .. 2R+3 as the pair budget allows - plus, on every other probed ring (all polar rings of both
+    hemispheres, band edges, seeded random rings), the phi positions of `seam_ks`; plus random pixels."""
     rng = np.random.default_rng(seed)
     nt, nph = w.n_theta, w.n_phi
-    rings = sorted(set(list(range(0, min(nt, 2 * plan_r + 4))) + list(range(max(0, nt - 2 * plan_r - 4), nt)) +
-                       [nt // 2 - 1, nt // 2, nt // 4, nt // 3] + [int(r) for r in rng.integers(0, nt, size=24)]))
-    ks = sorted(set([0, 1, 15, 16, 511, 512, 513, nph // 2 - 1, nph // 2, nph - 512, nph - 17, nph - 1] +
-                    [int(k) for k in rng.integers(0, nph, size=12)]))
-    pix = [r * nph + k for r in rings for k in ks if k < nph]
-    pix += [int(p) for p in rng.integers(0, nt * nph, size=n_random)]
-    return np.array(sorted(set(pix)), dtype=np.int64)
+    r = plan.work()[2]
+    fn = plan.info().first_narrow_ring
+    items = plan.items()
+    north_bands = sorted({(it[1], it[1] + it[2]) for it in items if it[0] == 1 and it[2] > 0})
+    whole, sampled = [], set()
+    if 0 < fn < (nt + 1) // 2:
+        whole += [fn, fn - 1, nt - 1 - fn, nt - fn]            # class boundary, both hemispheres
+    if len(north_bands) >= 2:
+        b = north_bands[len(north_bands) // 2]
+        whole += [b[0] - 1, b[0], nt - 1 - b[0]]                # last ring of a band / first of the next (+ south mirror)
+    whole += [nt // 2 - 1, nt // 2]
+    whole += list(range(0, min(nt, 2 * r + 4)))                 # polar rings, heaviest: taken while the budget lasts
+    for b in north_bands[:6]:
+        sampled |= {b[0], b[1] - 1, nt - 1 - b[0], nt - b[1]}
+    sampled |= set(range(0, min(nt, 2 * r + 4))) | set(range(max(0, nt - 2 * r - 4), nt))
+    sampled |= {nt // 4, nt // 3, fn + 1, max(0, fn - 2)} | {int(x) for x in rng.integers(0, nt, size=24)}
+    ks = seam_ks(nph, rng)
+    budget = ORACLE_PAIR_BUDGET - 2e8
+    pix, seen_whole = [], []
+    for i in whole:
+        if not (0 <= i < nt) or i in seen_whole:
+            continue
+        cost = ring_taps(plan, i, nt, nph, r) * nph
+        if cost > budget:
+            continue
+        budget -= cost
+        seen_whole.append(i)
+        pix += [i * nph + k for k in range(nph)]
+    for i in sorted(sampled):
+        if 0 <= i < nt and i not in seen_whole:
+            pix += [i * nph + k for k in ks]
+    pix += [int(p) for p in rng.integers(0, nt * nph, size=600)]
+    return np.array(sorted(set(pix)), dtype=np.int64), seen_whole
 
 
-FULL_SIZE = [(2, 0), (3, 0), (3, 3), (4, 0), (4, 2)]
+FULL_SIZE = [(2, 0), (3, 0), (3, 1), (3, 2), (3, 3), (4, 0), (4, 1), (4, 2), (4, 3)]
 
 
 @pytest.mark.parametrize("cfg,k", FULL_SIZE)
 def test_full_size_configs_on_sampled_pixels(torch, arkcos, cfg, k):
-    """BASELINE configs[2..4] at full size, in the launch configuration bench.py times; the oracle
-    evaluates sampled output pixels one by one."""
+    """Every workload of BASELINE configs[2..4] at full size, in the launch configuration bench.py times; the
+    oracle evaluates whole rings at the schedule's seams and sampled pixels elsewhere, one by one."""
     w = wl.config(cfg)[k]
     x32 = w.map_f32(); table = w.table()
     with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut) as plan:
-        r = plan.work()[2]
         d_in = torch.from_numpy(x32).cuda()
         d_out = torch.full_like(d_in, float("nan"))
         plan.convolve(d_in, d_out, torch.cuda.current_stream().cuda_stream)
         torch.cuda.synchronize()
         got_full = d_out.cpu().numpy()
+        pix, whole = probe_pixels(w, plan, 2000 + cfg * 10 + k)
     assert np.isfinite(got_full).all()
-    pix = sample_pixels(w, 600, 2000 + cfg * 10 + k, r)
+    assert len(whole) >= 3, whole
     expect = oracle.convolve(x32, table, w.theta_cut, level=1, pixels=pix)
     scale = math.sqrt((got_full.astype(np.float64) ** 2).mean())     # global output rms
-    assert_parity(got_full.reshape(-1)[pix], expect, scale_rms=scale, what=w.name)
+    assert_parity(got_full.reshape(-1)[pix], expect, scale_rms=scale, what=f"{w.name} (whole rings {whole})")
     # properties that hold at any size: phi-shift equivariance of the GPU operator itself
     shift = 1000
     with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=arkcos.PLAN_CACHE_WEIGHTS) as plan:
@@ -226,3 +276,78 @@ def test_full_size_configs_on_sampled_pixels(torch, arkcos, cfg, k):
         torch.cuda.synchronize()
         rolled = d_out.cpu().numpy()
     assert np.abs(rolled - np.roll(got_full, shift, axis=1)).max() <= 2e-6 * scale
+
+
+def test_config4_batch_of_8_maps(torch, arkcos):
+    """configs[4] as BASELINE states it: a batch of 8 maps (seeds 10-17) through arkcos_convolve_batch, each map
+    checked against the oracle on sampled pixels, and against a single-map arkcos_convolve bit for bit."""
+    w = wl.config(4)[0]
+    table = w.table()
+    maps = np.stack([w.map_f32(m) for m in range(8)])
+    rng = np.random.default_rng(4108)
+    with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut) as plan:
+        d_in = torch.from_numpy(maps).cuda()
+        d_out = torch.full_like(d_in, float("nan"))
+        plan.convolve_batch(d_in, d_out, 8, torch.cuda.current_stream().cuda_stream)
+        single = torch.full_like(d_in[5], float("nan"))
+        plan.convolve(d_in[5], single, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy()
+        assert torch.equal(single, d_out[5])
+        r = plan.work()[2]
+    assert np.isfinite(got).all()
+    ks = seam_ks(w.n_phi, rng)
+    rings = sorted(set(range(0, 2 * r + 4)) | {w.n_theta - 1, w.n_theta // 2, 1000, 3000} | {int(x) for x in rng.integers(0, w.n_theta, 8)})
+    pix = np.array(sorted({i * w.n_phi + k for i in rings for k in ks} | {int(p) for p in rng.integers(0, w.n_pix, 300)}), dtype=np.int64)
+    for m in range(8):
+        expect = oracle.convolve(maps[m], table, w.theta_cut, level=1, pixels=pix)
+        scale = math.sqrt((got[m].astype(np.float64) ** 2).mean())
+        assert_parity(got[m].reshape(-1)[pix], expect, scale_rms=scale, what=f"{w.name} map {m} (seed {w.map_seeds[m]})")
+
+
+def test_interleaved_plans_of_different_shared_memory_size(torch, arkcos):
+    """The dynamic shared-memory attribute belongs to the kernel, not to a plan: a small plan created
+    after a large one must not break the large one's launches, and vice versa."""
+    rng = np.random.default_rng(77)
+    big = (256, 2048, 2.1 * DEG)       # narrow band marching, R = 2: ~190 KB of dynamic shared memory
+    small = (16, 32, 7.0 * DEG)
+    tabs = {big: rng.standard_normal(64), small: rng.standard_normal(37)}
+    xs = {g: rng.standard_normal(g[:2]).astype(np.float32) for g in (big, small)}
+    expect = {g: oracle.convolve(xs[g], tabs[g], g[2], level=1) for g in (big, small)}
+    plans = []
+    try:
+        for g in (big, small, big, small):
+            plans.append((g, arkcos.Plan(g[0], g[1], tabs[g], g[2])))
+        for g, plan in plans + plans[::-1]:
+            d_in = torch.from_numpy(xs[g]).cuda()
+            d_out = torch.full_like(d_in, float("nan"))
+            plan.convolve(d_in, d_out, torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            assert_parity(d_out.cpu().numpy(), expect[g], what=f"interleaved plan {g}")
+    finally:
+        for _, plan in plans:
+            plan.destroy()
+
+
+def test_one_plan_on_two_streams_concurrently(torch, arkcos):
+    """a plan may be used concurrently from several streams.  On-the-fly plans rewrite the weight
+    buffer in every call with bit-identical values; calls interleaved on two non-blocking streams must give the
+    single-stream result bit for bit."""
+    w = wl.config(1)[0]
+    table = w.table()
+    maps = [wl.white_map(w.n_theta, w.n_phi, s) for s in (50, 51)]
+    with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut) as plan:
+        d_in = [torch.from_numpy(m).cuda() for m in maps]
+        ref = [torch.empty_like(d_in[0]) for _ in range(2)]
+        for m in range(2):
+            plan.convolve(d_in[m], ref[m], torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        outs = [[torch.full_like(d_in[0], float("nan")) for _ in range(6)] for _ in range(2)]
+        for rep in range(6):
+            for m in range(2):
+                plan.convolve(d_in[m], outs[m][rep], streams[m].cuda_stream)
+        torch.cuda.synchronize()
+        for m in range(2):
+            for rep in range(6):
+                assert torch.equal(outs[m][rep], ref[m]), (m, rep)

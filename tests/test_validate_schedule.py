@@ -1,0 +1,56 @@
+"""The host-side schedule validator (validate_schedule in csrc/arkcos_schedule.cpp).
+
+The kernels form addresses from the plan's descriptors without bounds checks, so plan creation re-derives,
+as plain integer arithmetic, every global range and shared-memory offset they will form and refuses to upload
+a schedule that fails (ARKCOS_EINTERNAL).  Here: (a) every BASELINE.json workload at FULL size validates,
+(b) the validator rejects each of ~30 single-field corruptions (tests/emu/validate_mutations.cpp)."""
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1211_3556_b200 import arkcos
+from paper_1211_3556_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+EMU_DIR = os.path.join(ROOT, "tests", "emu")
+CSRC = os.path.join(ROOT, "paper_1211_3556_b200", "csrc")
+
+
+@pytest.mark.parametrize("w", wl.all_workloads() + [wl.paper_regime_workload()], ids=lambda w: w.name)
+def test_every_full_size_workload_validates(w):
+    with arkcos.Plan(w.n_theta, w.n_phi, np.ones(8), w.theta_cut, flags=arkcos.PLAN_HOST_ONLY) as p:
+        status, why = p.validate()
+        assert status == arkcos.OK, why
+        info = p.info()
+        assert info.n_items > 0 and info.fma_slots >= info.pair_evals
+
+
+@pytest.mark.parametrize("n_theta,n_phi,cut_deg", [(1, 4, 10.0), (1, 4, 180.0), (2, 8, 95.0), (7, 12, 100.0), (10, 20, 180.0),
+                                                   (33, 64, 21.0), (20, 1028, 9.5), (5, 2052, 40.1), (12, 4100, 50.0),
+                                                   (301, 256, 3.69), (80, 2048, 4.3), (400, 8192, 1.3)])
+def test_odd_grids_validate(n_theta, n_phi, cut_deg):
+    with arkcos.Plan(n_theta, n_phi, np.ones(8), math.radians(cut_deg), flags=arkcos.PLAN_HOST_ONLY) as p:
+        status, why = p.validate()
+        assert status == arkcos.OK, why
+
+
+@pytest.fixture(scope="module")
+def mutations_bin(tmp_path_factory):
+    out = str(tmp_path_factory.mktemp("vm") / "validate_mutations")
+    cmd = ["g++", "-std=c++17", "-O1", "-g", "-fsanitize=address", "-I", CSRC, os.path.join(EMU_DIR, "validate_mutations.cpp"),
+           os.path.join(CSRC, "arkcos_schedule.cpp"), "-o", out]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr[-3000:]
+    return out
+
+
+@pytest.mark.parametrize("n_theta,n_phi,cut", [(64, 128, math.radians(9.0)), (4096, 8192, 15.0 * wl.ARCMIN),
+                                               (2048, 4096, 66.0 * wl.ARCMIN), (9, 16, math.radians(50.0)),
+                                               (4096, 8192, 5.0 * wl.ARCMIN)])
+def test_validator_rejects_every_single_field_corruption(mutations_bin, n_theta, n_phi, cut):
+    res = subprocess.run([mutations_bin, str(n_theta), str(n_phi), repr(cut)], capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    assert "mutations rejected" in res.stdout
