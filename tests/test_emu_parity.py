@@ -105,3 +105,27 @@ def test_emulated_two_phi_tiles_and_oscillating_kernel(emu_bin, tmp_path):
     rms = math.sqrt((expect ** 2).mean())
     assert not np.isnan(got).any(), log
     assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("n_theta,cut_deg,stride,expect_narrow", [(400, 1.3, 5, True), (96, 9.0, 3, False)])
+def test_emulated_launch_shapes_of_the_timed_configs(emu_bin, tmp_path, n_theta, cut_deg, stride, expect_narrow):
+    """n_phi = 8192, the ring length of configs[2] and configs[4]: WIDE items with F = 8 sub-tiles / S = 1, NARROW
+    items with the widest tile.  Every `stride`-th work item is run (EMU_ITEM_STRIDE); the outputs of the
+    skipped items stay NaN and only the written ones are compared.  An oscillating kernel, so a misplaced tap shows."""
+    import re
+    n_phi = 8192
+    cut = math.radians(cut_deg)
+    th = np.linspace(0.0, cut, 2048)
+    table = np.cos(5.0 * th / cut) * np.exp(-0.5 * (th / (0.45 * cut)) ** 2) * 30.0
+    x32 = np.random.default_rng(8192 + n_theta).standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut, env={"EMU_ITEM_STRIDE": str(stride)})
+    assert (int(re.search(r"items wide \d+ narrow (\d+)", log).group(1)) > 0) == expect_narrow, log
+    written = ~np.isnan(got)
+    rings = np.nonzero(written.any(axis=1))[0]
+    assert len(rings) >= 8 and written.mean() > 0.5 / stride, log
+    pix = np.flatnonzero(written.reshape(-1))
+    pix = pix[:: max(1, len(pix) // 60000)]                     # bounded oracle work
+    expect = oracle.convolve(x32, table, cut, level=1, pixels=pix)
+    full_rms = math.sqrt((expect ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / full_rms <= 1e-6 and float(np.abs(err).max()) / full_rms <= 1e-5, log
