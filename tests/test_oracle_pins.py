@@ -104,6 +104,24 @@ def test_level1_equals_level0_small_grid_any_cut(cut_deg):
     np.testing.assert_allclose(o1, o0, rtol=0, atol=1e-13 * max(1e-300, np.abs(o0).max()))
 
 
+def test_level1_equals_level0_at_planck_scale_polar_pixels():
+    """The acos window of level 1 (arkcos_oracle.c: pixel_level1) at configs[2]'s polar sin(theta) ~ 4e-4 and at the
+    configs[4]-40' cut, where (cos cut - cos t_i cos t_j)/(sin t_i sin t_j) is a ratio of two tiny numbers: level 1
+    must visit every in-support pair level 0 (ALL 33.5 M input pixels per output pixel) finds.  ~12 pixels x 2 cuts."""
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal((4096, 8192))
+    for w in (wl.config(2)[0], wl.config(4)[3]):
+        table = w.table()
+        r = int(w.theta_cut / (math.pi / w.n_theta))
+        rings = [0, 1, 2, r, r + 1, 2 * r + 3]
+        pix = np.array([i * w.n_phi + int(k) for i in rings for k in (0, int(rng.integers(1, w.n_phi)))][:6] +
+                       [(w.n_theta - 1) * w.n_phi + 7, (w.n_theta - 1 - r) * w.n_phi + 8191], dtype=np.int64)
+        o0, p0 = oracle.convolve(x, table, w.theta_cut, level=0, pixels=pix, return_pairs=True)
+        o1, p1 = oracle.convolve(x, table, w.theta_cut, level=1, pixels=pix, return_pairs=True)
+        assert p0 == p1 and p0 > 1e4 * len(pix)
+        np.testing.assert_allclose(o1, o0, rtol=0, atol=1e-13 * np.abs(o0).max())
+
+
 def test_pixel_subset_matches_full_map():
     w = wl.config(0)[0]
     x, table = w.map(), w.table()
@@ -239,9 +257,10 @@ def test_table_doubling_changes_result_at_second_order():
     assert 2.5 < e[0] / e[1] < 5.5 and 2.5 < e[1] / e[2] < 5.5   # ~4x per doubling (discrete gammas: not exactly 4)
 
 
-def test_support_is_inclusive_at_exact_ring_spacing():
-    """theta_cut exactly 2 ring spacings on the same meridian: gamma == theta_cut up to rounding is
-    ambiguous in FP, so test just inside/outside instead."""
+def test_support_edge_is_sharp_around_exact_ring_spacing():
+    """theta_cut just inside / just outside 2 ring spacings on the same meridian: the support is a sharp disc.
+    This does NOT tell `<` from `<=`: gamma == theta_cut exactly is decided by FP64 rounding of the unit vectors,
+    not by the method (R3), and no config has a tap within 1e-7 of the cut."""
     nt, nph = 18, 36
     dth = math.pi / nt
     table = np.ones(8)
