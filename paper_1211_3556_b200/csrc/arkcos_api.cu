@@ -47,7 +47,7 @@ struct arkcos_plan {
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging (arkcos_plan_reserve_host_io)
     size_t device_bytes = 0;
-    size_t conv_smem = 0, gen_smem = 0;
+    size_t gen_smem = 0;
     int gen_grid = 0, table_in_smem = 0;
 };
 
@@ -81,16 +81,26 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
     return ARKCOS_OK;
 }
 
+// S3 / S3w: the WIDE items (k_convolve_wide, one CTA per SM) and the NARROW items (k_convolve_narrow, two CTAs per
+// SM) of the plan, back to back on the caller's stream.  The two kernels write disjoint output rings.
 arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
+    const Schedule& s = pl->sched;
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
-    c.runs = pl->d_runs; c.first_narrow = pl->sched.first_narrow; c.narrow_w_base = pl->sched.narrow_w_base;
-    c.n_theta = pl->sched.n_theta; c.n_phi = pl->sched.n_phi; c.R = pl->sched.R; c.wslot = pl->sched.narrow_wslot;
-    c.map_stride = (long long)pl->sched.n_theta * pl->sched.n_phi;
-    if (pl->sched.items.empty()) return ARKCOS_OK;
-    dim3 grid((unsigned)pl->sched.items.size(), (unsigned)n_maps, 1);
-    k_convolve<<<grid, kThreads, pl->conv_smem, st>>>(c);
-    CU(cudaGetLastError());
+    c.runs = pl->d_runs; c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
+    c.n_theta = s.n_theta; c.n_phi = s.n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
+    c.map_stride = (long long)s.n_theta * s.n_phi;
+    const int n_wide = (pl->flags & ARKCOS_PLAN_ONLY_NARROW) ? 0 : s.n_wide_items;
+    const int n_narrow = (pl->flags & ARKCOS_PLAN_ONLY_WIDE) ? 0 : (int)s.items.size() - s.n_wide_items;
+    if (n_wide > 0) {
+        k_convolve_wide<<<dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, s.smem_wide, st>>>(c);
+        CU(cudaGetLastError());
+    }
+    if (n_narrow > 0) {
+        c.items = pl->d_items + s.n_wide_items;
+        k_convolve_narrow<<<dim3((unsigned)n_narrow, (unsigned)n_maps, 1), kThreads, s.smem_narrow, st>>>(c);
+        CU(cudaGetLastError());
+    }
     return ARKCOS_OK;
 }
 
@@ -176,13 +186,6 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         }
         int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
         if (rc != 0) { delete pl; return (arkcos_status)rc; }
-        if (pl->sched.smem_bytes > (size_t)kSmemBudget) { delete pl; return ARKCOS_EUNSUPPORTED; }
-        if (flags & (ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) {     // measurement hooks
-            const int keep = (flags & ARKCOS_PLAN_ONLY_WIDE) ? kWide : kNarrow;
-            std::vector<Item> kept;
-            for (const Item& it : pl->sched.items) if (it.kind == keep) kept.push_back(it);
-            pl->sched.items.swap(kept);
-        }
     } catch (const std::bad_alloc&) { delete pl; return ARKCOS_ENOMEM; }
     if (flags & ARKCOS_PLAN_HOST_ONLY) { *plan = pl; return ARKCOS_OK; }
 
@@ -208,9 +211,10 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         // launch configuration.  The dynamic shared-memory limit is an attribute of the KERNEL, shared by every
         // plan of the process: always set it to the library's maximum, never to this plan's own size (a later,
         // smaller plan must not lower it under an earlier plan's launches).
-        pl->conv_smem = s.smem_bytes;
-        if (!cuda_ok(cudaFuncSetAttribute(k_convolve, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
-                     "cudaFuncSetAttribute(k_convolve)")) { st = ARKCOS_ECUDA; break; }
+        if (!cuda_ok(cudaFuncSetAttribute(k_convolve_wide, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
+                     "cudaFuncSetAttribute(k_convolve_wide)") ||
+            !cuda_ok(cudaFuncSetAttribute(k_convolve_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
+                     "cudaFuncSetAttribute(k_convolve_narrow)")) { st = ARKCOS_ECUDA; break; }
         size_t tab_bytes = (size_t)n_table * sizeof(double);
         pl->table_in_smem = tab_bytes <= (size_t)kGenSmemMax ? 1 : 0;
         pl->gen_smem = pl->table_in_smem ? tab_bytes : 0;
@@ -327,7 +331,11 @@ arkcos_status arkcos_plan_get_info(const arkcos_plan* pl, arkcos_plan_info* info
     info->ring_halfband = s.R; info->pair_evals = s.pair_evals; info->weights = s.weights;
     info->fma_slots = s.fma_slots; info->weight_slots = s.weight_slots;
     info->n_items = (int)s.items.size(); info->n_gen_units = (int)s.gen_units.size();
-    info->kernels_per_convolve = (pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) ? 1 : 2;
+    {
+        const int n_wide = (pl->flags & ARKCOS_PLAN_ONLY_NARROW) ? 0 : s.n_wide_items;
+        const int n_narrow = (pl->flags & ARKCOS_PLAN_ONLY_WIDE) ? 0 : (int)s.items.size() - s.n_wide_items;
+        info->kernels_per_convolve = ((pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) ? 0 : 1) + (n_wide > 0) + (n_narrow > 0);
+    }
     info->sm_count = pl->sm_count; info->flags = pl->flags; info->device_bytes = pl->device_bytes;
     info->fma_slots_wide = s.fma_slots_wide; info->first_narrow_ring = s.first_narrow;
     return ARKCOS_OK;
@@ -336,8 +344,9 @@ arkcos_status arkcos_plan_get_info(const arkcos_plan* pl, arkcos_plan_info* info
 arkcos_status arkcos_plan_item(const arkcos_plan* pl, int index, int* fields) {
     if (!pl || !fields || index < 0 || index >= (int)pl->sched.items.size()) return ARKCOS_EINVAL;
     const Item& it = pl->sched.items[index];
-    fields[0] = it.kind; fields[1] = it.i0; fields[2] = it.nrings; fields[3] = it.k0; fields[4] = kWarpSpan << it.f_log2;
-    fields[5] = kWarps >> it.f_log2;
+    fields[0] = it.kind; fields[1] = it.i0; fields[2] = it.nrings; fields[3] = it.k0;
+    fields[4] = it.kind == kWide ? kWarpSpan << it.f_log2 : kNarrowSpan;
+    fields[5] = it.kind == kWide ? kWarps >> it.f_log2 : kWarps;
     return ARKCOS_OK;
 }
 

@@ -30,10 +30,15 @@ constexpr int kSmemBudget = 220 * 1024;
 // 144 bytes) are bank-conflict free.  Logical 16-byte chunk c sits at physical chunk c + (c >> 3).
 constexpr int kTileBytes = 144;
 
-// ---- NARROW items: band marching -----------------------------------------------------------------
-// Row slot = left halo tile + F * 32 own tiles + right halo tile + one spare tile (software prefetch
-// of the sliding window reads at most one tile past the right halo).
-ARKCOS_HD constexpr int narrow_slot_bytes(int f_log2) { return ((32 << f_log2) + 3) * kTileBytes; }
+// ---- NARROW items: band marching, kNarrowP outputs per lane ----------------------------------------
+// A warp owns kNarrowSpan contiguous outputs of one ring; a lane's tile is kNarrowP floats = 4 chunks of 16
+// bytes + 1 pad chunk (lane stride 80 bytes: the 16-byte window loads of a warp are bank-conflict free).
+// Row slot = 2 left halo tiles + 32 own tiles + 2 right halo tiles + one spare tile (the software prefetch of
+// the sliding window reads at most one tile past the right halo).
+constexpr int kNarrowP = 16;
+constexpr int kNarrowSpan = 32 * kNarrowP;           // 512 contiguous phi outputs per warp = per NARROW item
+constexpr int kNarrowTileBytes = 80;
+constexpr int kNarrowSlotBytes = (32 + 2 * (kHaloNarrow / kNarrowP) + 1) * kNarrowTileBytes;
 
 // ---- WIDE items (windows of 64 .. n_phi taps): warp-autonomous path ------------------------------
 // A warp owns kWarpSpan contiguous outputs of ONE ring and streams its share of the ring's taps through
@@ -72,8 +77,9 @@ struct Item {
     int32_t i0;       // kWide: the output ring (either hemisphere).  kNarrow: first NORTHERN output ring
                       //   (the CTA also produces the mirror rings)
     int32_t k0;       // first output phi of the tile
-    int16_t f_log2;   // F = 1 << f_log2 phi sub-tiles of kWarpSpan outputs; S = kWarps / F
-    int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings, S rings per pass
+    int16_t f_log2;   // kWide: F = 1 << f_log2 phi sub-tiles of kWarpSpan outputs; S = kWarps / F.  kNarrow: 0
+                      //   (the tile is kNarrowSpan outputs; kWarps rings per pass)
+    int16_t kind;     // kWide: one ring, S tap splits.  kNarrow: `nrings` rings
     int32_t nrings;   // kNarrow: rings of the band; negative = the band is the southern mirror of
                       //   northern rings [i0, i0 - nrings)
     int32_t wcopy;    // kNarrow: floats of a ring's weight block to stage (max over the band; multiple of 4)
@@ -107,12 +113,12 @@ struct Schedule {
     uint32_t narrow_w_base = 0;             // weights of narrow ring i start at narrow_w_base + (i - first_narrow) * narrow_wslot
     std::vector<uint32_t> ring_w_off;       // [n_north] offset of the ring's (contiguous) weights
     std::vector<uint32_t> ring_slots;       // [n_north] stored taps of the ring (sum over rows, padded to 4)
-    std::vector<Item> items;                // cost-sorted, heaviest first
+    std::vector<Item> items;                // the WIDE items, then the NARROW items; each part cost-sorted, heaviest first
+    int n_wide_items = 0;                   // items[0 .. n_wide_items) are WIDE (kernel k_convolve_wide), the rest NARROW
     std::vector<GenUnit> gen_units;
     int first_narrow = 0;                   // rings [first_narrow, n_north) use the narrow kernel path
-    int narrow_f_log2 = 0;                  // F of the narrow items
     int narrow_wslot = 0;                   // floats per ring in the narrow weight buffers
-    size_t smem_bytes = 0;                  // dynamic shared memory of the convolution launch
+    size_t smem_wide = 0, smem_narrow = 0;  // dynamic shared memory of the two convolution kernels
     unsigned long long pair_evals = 0;      // useful FMAs per map
     unsigned long long weights = 0;         // in-support weights, no symmetry reduction
     unsigned long long fma_slots = 0;       // FMA lanes issued per map (padding included)
@@ -130,7 +136,7 @@ struct Schedule {
 
 // shared memory of a WIDE item (two private stage buffers per warp), and of the NARROW path
 size_t wide_smem_bytes(int R);
-size_t narrow_smem_bytes(int f_log2, int R, int wslot);
+size_t narrow_smem_bytes(int R, int wslot);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
 int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);

@@ -93,14 +93,15 @@ __global__ void __launch_bounds__(kGenThreads) k_generate_weights(const GenParam
 //                streams its share of the ring's taps through private double-buffered stages.
 //   NARROW items (windows inside [-32, 32)): a band of rings of one hemisphere marches through a
 //                shared-memory ring of 2R+2S input rows, S rings per pass, so every input row is
-//                staged once per band; the window loads of a row use immediate offsets only.
+//                staged once per band; the window loads of a row use immediate offsets only; a lane
+//                owns kNarrowP = 16 outputs so that two CTAs fit an SM (kernel k_convolve_narrow).
 // Southern rings use the weights of their northern mirror (A_j and sin t are N/S symmetric).
 // ================================================================================================
 struct ConvParams {
     const float* in;
     float* out;
     const PairDesc* pairs;
-    const Item* items;
+    const Item* items;       // the items of THIS launch (the wide or the narrow part of the work list)
     const float* weights;
     const NarrowRun* runs;   // [n_north - first_narrow][2R+1]
     int n_theta, n_phi, R;
@@ -345,64 +346,59 @@ __device__ void conv_wide(const ConvParams& p, const Item& it, char* smem, const
 }
 
 // ------------------------------------------------------------------------------------------------
-// NARROW item: band marching.
+// NARROW item: band marching (kernel v5: 16 outputs per lane, two CTAs per SM).
 //
-// Window geometry of one (ring, input row) run.  The origin of the tap axis is d = -32, i.e. the
-// start of the tile to the LEFT of the lane's own tile; everything is counted in float PAIRS
-// (8 bytes): step K handles taps d = -32 + 2K and d + 1 and needs pairs K .. K+16 of the row.
-// A run enters the fully unrolled chain of 32 steps at K0 = (32 + start) / 2 and leaves it after
-// ntaps / 2 steps, so every shared-memory offset below is a compile-time immediate.
+// A (ring, input row) run of the narrow class is only 6 .. 32 taps long, so what limits it is not the FFMA
+// rate of its inner loop but the latency of its start (descriptor, jump table, window loads); v4 ran it with 32
+// outputs per lane in 8 warps per SM and reached 35 % of the FP32 peak (ncu: issue slots 59 % busy, stalls
+// wait / short scoreboard / no instruction).  v5 halves the lane's outputs (kNarrowP = 16): 80 instead of 151
+// registers and half the shared memory per CTA, so TWO CTAs (16 warps) are resident per SM and cover each
+// other's run starts; the unrolled chain shrinks from 35 KB to 18 KB (fits the 32 KB instruction cache level).
+//
+// Window geometry.  The origin of the tap axis is d = -32 = the start of the tile TWO to the left of the
+// lane's own tile (a tile = 16 floats = 4 chunks of 16 bytes, + 1 pad chunk in shared memory).  Step K handles
+// taps d = -32 + 2K and d + 1 and needs floats [2K, 2K + 16] of the row = chunks (K >> 1) .. (K >> 1) + 4.
+// The register window is a ring of 6 chunks (5 live + 1 prefetched by every EVEN step, two steps ahead of its
+// first use, as one conflict-free LDS.128).  A run enters the fully unrolled chain of 32 steps at
+// k0 = (32 + start) / 2 and leaves it after ntaps / 2 steps: every shared-memory offset is an immediate.
 // ------------------------------------------------------------------------------------------------
-constexpr int kNarrowPairs = 18;          // register window: 18 pairs = 36 floats (17 live + 1 prefetched)
+constexpr int kNarrowRing = 6;            // chunks of the register window
 constexpr int kNarrowSteps = kHaloNarrow; // steps of the chain (2 taps each)
 
-// byte offset of pair P (origin = pair 0 of the left neighbour tile) relative to the lane's own tile
-__host__ __device__ constexpr int narrow_pair_off(int P) {
-    const int v = (P >> 1) - 8;                                 // chunk relative to the own tile
-    const int tile = (v >= 0) ? v / 8 : -((-v + 7) / 8);        // floor(v / 8)
-    return 16 * (v + tile) + 8 * (P & 1);
+// byte offset of chunk q of the tap axis relative to the lane's own tile
+__host__ __device__ constexpr int narrow_chunk_off(int q) { return ((q >> 2) - 2) * kNarrowTileBytes + (q & 3) * 16; }
+
+template <int Q>
+__device__ __forceinline__ void narrow_load_chunk(float (&z)[4 * kNarrowRing], const uint32_t zt) {
+    constexpr int sl = 4 * (Q % kNarrowRing);
+    lds128i<narrow_chunk_off(Q)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt);
 }
 
 template <int K>
-__device__ __forceinline__ void narrow_init(float (&z)[2 * kNarrowPairs], float (&w)[2][2], const uint32_t zt, const uint32_t wq) {
-    constexpr int P0 = K + (K & 1);                             // first even pair
-    if constexpr ((K & 1) != 0) lds64i<narrow_pair_off(K)>(z[2 * (K % kNarrowPairs)], z[2 * (K % kNarrowPairs) + 1], zt);
-#pragma unroll
-    for (int c = 0; c < 8; c++) {
-        // pairs P0 + 2c, P0 + 2c + 1 share a 16-byte chunk; their ring slots are consecutive (18 is even)
-        const int sl = 2 * ((P0 + 2 * c) % kNarrowPairs);
-        switch (c) {   // the offset must be an immediate: one case per c
-            case 0: lds128i<narrow_pair_off(P0 + 0)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 1: lds128i<narrow_pair_off(P0 + 2)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 2: lds128i<narrow_pair_off(P0 + 4)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 3: lds128i<narrow_pair_off(P0 + 6)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 4: lds128i<narrow_pair_off(P0 + 8)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 5: lds128i<narrow_pair_off(P0 + 10)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            case 6: lds128i<narrow_pair_off(P0 + 12)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-            default: lds128i<narrow_pair_off(P0 + 14)>(z[sl], z[sl + 1], z[sl + 2], z[sl + 3], zt); break;
-        }
-    }
-    if constexpr ((K & 1) == 0) lds64i<narrow_pair_off(K + 16)>(z[2 * ((K + 16) % kNarrowPairs)], z[2 * ((K + 16) % kNarrowPairs) + 1], zt);
+__device__ __forceinline__ void narrow_init(float (&z)[4 * kNarrowRing], float (&w)[2][2], const uint32_t zt, const uint32_t wq) {
+    constexpr int C = K >> 1;
+    narrow_load_chunk<C>(z, zt); narrow_load_chunk<C + 1>(z, zt); narrow_load_chunk<C + 2>(z, zt);
+    narrow_load_chunk<C + 3>(z, zt); narrow_load_chunk<C + 4>(z, zt);
+    if constexpr ((K & 1) != 0) narrow_load_chunk<C + 5>(z, zt);   // an odd entry step is followed by an even one that needs it
     lds64i<8 * K>(w[K & 1][0], w[K & 1][1], wq);
 }
 
 template <int K>
-__device__ __forceinline__ void narrow_step(float (&a0)[kLaneP], float (&a1)[kLaneP], float (&z)[2 * kNarrowPairs], float (&w)[2][2],
+__device__ __forceinline__ void narrow_step(float (&a0)[kNarrowP], float (&a1)[kNarrowP], float (&z)[4 * kNarrowRing], float (&w)[2][2],
                                             const uint32_t zt, const uint32_t wq) {
-    constexpr int N = 2 * ((K + 17) % kNarrowPairs);
-    lds64i<narrow_pair_off(K + 17)>(z[N], z[N + 1], zt);
+    if constexpr ((K & 1) == 0) narrow_load_chunk<(K >> 1) + 5>(z, zt);   // first used by step K + 2
     lds64i<8 * (K + 1)>(w[(K + 1) & 1][0], w[(K + 1) & 1][1], wq);
 #pragma unroll
-    for (int m = 0; m < kLaneP; m++) a0[m] = fmaf(z[(2 * K + m) % (2 * kNarrowPairs)], w[K & 1][0], a0[m]);
+    for (int m = 0; m < kNarrowP; m++) a0[m] = fmaf(z[(2 * K + m) % (4 * kNarrowRing)], w[K & 1][0], a0[m]);
 #pragma unroll
-    for (int m = 0; m < kLaneP; m++) a1[m] = fmaf(z[(2 * K + m + 1) % (2 * kNarrowPairs)], w[K & 1][1], a1[m]);
+    for (int m = 0; m < kNarrowP; m++) a1[m] = fmaf(z[(2 * K + m + 1) % (4 * kNarrowRing)], w[K & 1][1], a1[m]);
 }
 
-// a0[m] + a1[m] += sum_{e < 2 n} wrow[e] * Z[m + 2 k0 + e],  Z = the row from the start of the left neighbour tile.
+// a0[m] + a1[m] += sum_{e < 2 n} wrow[e] * Z[m + 2 k0 + e],  Z = the row from the start of the tile two to the left.
 // zt: shared address of the lane's own tile in the row slot; wq = address of wrow - 8 k0 bytes.
 #pragma nv_diag_suppress 177   // the chain's labels past K = 16 are only fallen into
-__device__ __forceinline__ void narrow_row(float (&a0)[kLaneP], float (&a1)[kLaneP], const uint32_t zt, const uint32_t wq, const int k0, int n) {
-    float z[2 * kNarrowPairs];
+__device__ __forceinline__ void narrow_row(float (&a0)[kNarrowP], float (&a1)[kNarrowP], const uint32_t zt, const uint32_t wq, const int k0, int n) {
+    float z[4 * kNarrowRing];
     float w[2][2];
 #define ARKCOS_NR_CASE(K) case K: narrow_init<K>(z, w, zt, wq); goto nr_step_##K;
 #define ARKCOS_NR_STEP(K) nr_step_##K: narrow_step<K>(a0, a1, z, w, zt, wq); if (--n == 0) goto nr_done;
@@ -424,17 +420,19 @@ nr_done:;
 }
 #pragma nv_diag_default 177
 
-// A band of `nr` rings of one hemisphere, in "logical" (northern) ring indices lam: the physical ring of
-// logical ring lam is lam (north) or n_theta-1-lam (south); descriptors and weights are those of lam.
+// A band of `nr` rings of one hemisphere x a phi tile of kNarrowSpan outputs, in "logical" (northern) ring
+// indices lam: the physical ring of logical ring lam is lam (north) or n_theta-1-lam (south); descriptors and
+// weights are those of lam.  The band marches through a shared-memory ring of 2R + 2S row slots, S = kWarps rings
+// per pass (one warp per ring), so every input row is staged once per band; the S rows, the weight blocks and
+// the run descriptors of the NEXT pass are copied by cp.async during the current pass (one barrier per pass).
 __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, const float* in, float* out) {
-    const int F = 1 << it.f_log2, S = kWarps >> it.f_log2;
+    constexpr int S = kWarps;
     const bool south = it.nrings < 0;
     const int nr = south ? -it.nrings : it.nrings;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int f = warp & (F - 1), s = warp >> it.f_log2;
+    const int s = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int W = 2 * p.R + 1;
     const int NS = 2 * p.R + 2 * S;                           // row slots
-    const int slot_bytes = narrow_slot_bytes(it.f_log2);
+    constexpr int slot_bytes = kNarrowSlotBytes;
     const uint32_t rows = (uint32_t)__cvta_generic_to_shared(smem);
     float* wbuf = reinterpret_cast<float*>(smem + (size_t)NS * slot_bytes);               // [2][S][wslot]
     NarrowRun* pdbuf = reinterpret_cast<NarrowRun*>(wbuf + 2 * (size_t)S * p.wslot);      // [2][S][W]
@@ -443,23 +441,17 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     const int lam0 = it.i0, lam_end = it.i0 + nr;
     const int npass = (nr + S - 1) / S;
 
-    // ---- row staging: chunk idx of a row slot = floats [4 idx, 4 idx + 4) from phi = k0 - 32 ------------
-    const int row_chunks = ((32 << it.f_log2) + 2) * 8;       // halo + own tiles + halo
-    const int t_phi0 = wrap_phi(it.k0 - kHaloNarrow + 4 * (int)threadIdx.x, p.n_phi);
-    const int t_phi_step = (4 * kThreads) % p.n_phi;
-    const uint32_t t_dst0 = (uint32_t)((threadIdx.x + (threadIdx.x >> 3)) << 4);
+    // ---- row staging: chunk idx of a row slot = floats [4 idx, 4 idx + 4) from phi = k0 - 32; tile = 4 chunks + pad ----
+    constexpr int row_chunks = kNarrowSpan / 4 + 2 * (kHaloNarrow / 4);     // own tiles + a halo of 32 floats on either side
+    static_assert(row_chunks <= kThreads, "one cp.async per thread stages a row");
+    const int t_phi = wrap_phi(it.k0 - kHaloNarrow + 4 * (int)threadIdx.x, p.n_phi);
+    const uint32_t t_dst = (uint32_t)((threadIdx.x + (threadIdx.x >> 2)) << 4);
     auto stage_row = [&](const int lam_j) {
         if (lam_j < 0 || lam_j >= p.n_theta) return;          // beyond the pole: no ring pair uses it
+        if ((int)threadIdx.x >= row_chunks) return;
         const float* row = in + (size_t)(south ? p.n_theta - 1 - lam_j : lam_j) * p.n_phi;
         int sl = lam_j % NS; if (sl < 0) sl += NS;
-        uint32_t dst = rows + (uint32_t)(sl * slot_bytes) + t_dst0;
-        int phi = t_phi0;
-        for (int idx = threadIdx.x; idx < row_chunks; idx += kThreads) {
-            cp_async16(dst, row + phi);
-            dst += (kThreads + kThreads / 8) * 16;
-            phi += t_phi_step;
-            if (phi >= p.n_phi) phi -= p.n_phi;
-        }
+        cp_async16(rows + (uint32_t)(sl * slot_bytes) + t_dst, row + t_phi);
     };
     // weights and run descriptors of the S rings of a pass -> buffer b (no dependent global loads:
     // both live at computable addresses)
@@ -479,7 +471,7 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     for (int lam_j = lam0 - p.R; lam_j < lam0 + S + p.R; lam_j++) stage_row(lam_j);
     stage_ring_tables(0, 0);
 
-    const uint32_t lane_tile = (uint32_t)((1 + f * 32 + lane) * kTileBytes);
+    const uint32_t lane_tile = (uint32_t)((kHaloNarrow / kNarrowP + lane) * kNarrowTileBytes);
     for (int pass = 0; pass < npass; pass++) {
         const int lbase = lam0 + pass * S;
         cp_async_wait_all();
@@ -490,9 +482,9 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
         }
         const int lam = lbase + s;
         if (lam < lam_end) {
-            float a0[kLaneP], a1[kLaneP];
+            float a0[kNarrowP], a1[kNarrowP];
 #pragma unroll
-            for (int m = 0; m < kLaneP; m++) { a0[m] = 0.f; a1[m] = 0.f; }
+            for (int m = 0; m < kNarrowP; m++) { a0[m] = 0.f; a1[m] = 0.f; }
             const int tb = (pass & 1) * S + s;
             const uint32_t wring = wbuf_addr + (uint32_t)(tb * p.wslot * 4);
             const uint32_t spd = pdbuf_addr + (uint32_t)(tb * W * sizeof(NarrowRun));
@@ -513,10 +505,10 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
                 zt += (uint32_t)slot_bytes;
                 if (zt == zt_end) zt -= (uint32_t)(NS * slot_bytes);
             }
-            const int phi = it.k0 + f * kWarpSpan + lane * kLaneP;
+            const int phi = it.k0 + lane * kNarrowP;
             float* orow = out + (size_t)(south ? p.n_theta - 1 - lam : lam) * p.n_phi + phi;
 #pragma unroll
-            for (int g = 0; g < kLaneP / 4; g++)
+            for (int g = 0; g < kNarrowP / 4; g++)
                 if (phi + 4 * g < p.n_phi)
                     *reinterpret_cast<float4*>(orow + 4 * g) = make_float4(a0[4 * g] + a1[4 * g], a0[4 * g + 1] + a1[4 * g + 1],
                                                                            a0[4 * g + 2] + a1[4 * g + 2], a0[4 * g + 3] + a1[4 * g + 3]);
@@ -524,7 +516,10 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     }
 }
 
-__global__ void __launch_bounds__(kThreads, 1) k_convolve(const ConvParams p) {
+// ---- the two convolution kernels of a launch: WIDE items (1 CTA of 8 warps per SM), NARROW items (2 per SM) ----
+// The descriptors were validated on the host (validate_schedule) before they were uploaded; the guards only keep
+// a work item that was corrupted in device memory from being turned into addresses.
+__global__ void __launch_bounds__(kThreads, 1) k_convolve_wide(const ConvParams p) {
 #ifndef ARKCOS_HOST_EMU
     extern __shared__ uint4 smem4[];
     char* smem = reinterpret_cast<char*>(smem4);
@@ -532,14 +527,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_convolve(const ConvParams p) {
     char* smem = reinterpret_cast<char*>(emu::g_smem);
 #endif
     const Item it = p.items[blockIdx.x];
-    // The descriptors were validated on the host (validate_schedule) before they were uploaded; this guard only
-    // keeps a work item that was corrupted in device memory from being turned into addresses.
-    if ((unsigned)it.f_log2 > 3u || (unsigned)it.k0 >= (unsigned)p.n_phi || (unsigned)it.i0 >= (unsigned)p.n_theta ||
-        (it.kind != kWide && it.kind != kNarrow)) return;
-    const float* in = p.in + (long long)blockIdx.y * p.map_stride;
-    float* out = p.out + (long long)blockIdx.y * p.map_stride;
-    if (it.kind == kWide) conv_wide(p, it, smem, in, out);
-    else conv_narrow(p, it, smem, in, out);
+    if ((unsigned)it.f_log2 > 3u || (unsigned)it.k0 >= (unsigned)p.n_phi || (unsigned)it.i0 >= (unsigned)p.n_theta || it.kind != kWide) return;
+    conv_wide(p, it, smem, p.in + (long long)blockIdx.y * p.map_stride, p.out + (long long)blockIdx.y * p.map_stride);
+}
+
+__global__ void __launch_bounds__(kThreads, 2) k_convolve_narrow(const ConvParams p) {
+#ifndef ARKCOS_HOST_EMU
+    extern __shared__ uint4 smem4[];
+    char* smem = reinterpret_cast<char*>(smem4);
+#else
+    char* smem = reinterpret_cast<char*>(emu::g_smem);
+#endif
+    const Item it = p.items[blockIdx.x];
+    if ((unsigned)it.k0 >= (unsigned)p.n_phi || (unsigned)it.i0 >= (unsigned)p.n_theta || it.kind != kNarrow || it.nrings == 0) return;
+    conv_narrow(p, it, smem, p.in + (long long)blockIdx.y * p.map_stride, p.out + (long long)blockIdx.y * p.map_stride);
 }
 
 }  // namespace arkcos

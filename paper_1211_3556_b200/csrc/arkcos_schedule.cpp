@@ -126,21 +126,25 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             const PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half >= 0) narrow_range(p.half, nw_start[(size_t)i * W + r], nw_ntaps[(size_t)i * W + r]);
         }
+    // Band marching keeps 2R + 2 kWarps row slots and two buffers of kWarps ring weight blocks in shared memory.
+    // The weight block of a ring grows towards the pole: shrink the narrow class from its polar end until the
+    // launch fits (for a large ring band, R > ~25, nothing fits and every ring takes the WIDE path).
     {
-        unsigned long long wslot = 0;
-        for (int i = s.first_narrow; i < s.n_north; i++) {
-            unsigned long long slots = 0;
-            for (int r = 0; r < W; r++) slots += (unsigned long long)nw_ntaps[(size_t)i * W + r];
-            wslot = std::max(wslot, slots);
+        std::vector<unsigned long long> slots(s.n_north, 0);
+        for (int i = s.first_narrow; i < s.n_north; i++)
+            for (int r = 0; r < W; r++) slots[i] += (unsigned long long)nw_ntaps[(size_t)i * W + r];
+        for (;;) {
+            unsigned long long wslot = 0;
+            for (int i = s.first_narrow; i < s.n_north; i++) wslot = std::max(wslot, slots[i]);
+            s.narrow_wslot = (int)((wslot + 3) & ~3ull);
+            if (s.first_narrow >= s.n_north || narrow_smem_bytes(s.R, s.narrow_wslot) <= (size_t)kSmemBudget) break;
+            // drop the rings whose block is the largest (the polar end), at least one ring
+            int fn = s.first_narrow + 1;
+            while (fn < s.n_north && slots[fn] + 16 > wslot) fn++;
+            s.first_narrow = fn;
         }
-        s.narrow_wslot = (int)((wslot + 3) & ~3ull);
+        if (s.first_narrow >= s.n_north) { s.first_narrow = s.n_north; s.narrow_wslot = 0; }
     }
-    int nf_cap = 0;                                           // largest useful F of the narrow tiles
-    while (nf_cap < 3 && (kWarpSpan << nf_cap) < n_phi) nf_cap++;
-    s.narrow_f_log2 = -1;
-    for (int fl = nf_cap; fl >= 0; fl--)
-        if (narrow_smem_bytes(fl, s.R, s.narrow_wslot) <= (size_t)kSmemBudget) { s.narrow_f_log2 = fl; break; }
-    if (s.narrow_f_log2 < 0 || s.n_north - s.first_narrow < 1) { s.first_narrow = s.n_north; s.narrow_f_log2 = 0; }
 
     // ---- weight layout ------------------------------------------------------------------------------
     // WIDE rings: one contiguous block per ring.  NARROW rings: blocks at a uniform stride of narrow_wslot
@@ -203,11 +207,10 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     for (int i = 0; i < s.n_north; i++) total += ring_slots[i] * (unsigned long long)n_phi * (2 * i + 1 == n_theta ? 1ull : 2ull);
     const double c_max = (double)total / (double)sm_count / 8.0;   // no item above 1/8 of an SM's share, if possible
     struct Tmp { Item it; double cost; };
-    std::vector<Tmp> tmp;
-    size_t smem = 0;
+    std::vector<Tmp> tmp_wide, tmp_narrow;
     // WIDE: (ring of either hemisphere, phi tile of F sub-tiles of kWarpSpan outputs); S = 8/F tap splits
     if (s.first_narrow > 0) {
-        smem = std::max(smem, wide_smem_bytes(s.R));
+        s.smem_wide = wide_smem_bytes(s.R);
         int wf_cap = 0;
         while (wf_cap < 3 && (kWarpSpan << wf_cap) < n_phi) wf_cap++;
         for (int i = 0; i < s.first_narrow; i++) {
@@ -219,22 +222,23 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
                 const int valid = std::min(L, n_phi - k0);
                 const double cost = (double)ring_slots[i] * (double)valid + 4000.0;
                 for (int hemi = 0; hemi < (i_s != i ? 2 : 1); hemi++) {
-                    tmp.push_back(Tmp{Item{hemi ? i_s : i, k0, (int16_t)fl, (int16_t)kWide, 1, 0}, cost});
+                    tmp_wide.push_back(Tmp{Item{hemi ? i_s : i, k0, (int16_t)fl, (int16_t)kWide, 1, 0}, cost});
                     s.fma_slots += ring_slots[i] * (unsigned long long)L;
                     s.fma_slots_wide += ring_slots[i] * (unsigned long long)L;
                 }
             }
         }
     }
-    // NARROW: (band of B rings of one hemisphere, phi tile of F * kWarpSpan outputs); S = 8/F rings advance together
+    // NARROW: (band of B rings of one hemisphere, phi tile of kNarrowSpan outputs); kWarps rings advance together.
+    // Two CTAs share an SM, so a band is cut at half the WIDE items' cost cap.
     if (s.first_narrow < s.n_north) {
-        const int fl = s.narrow_f_log2, S = kWarps >> fl, L = kWarpSpan << fl;
-        smem = std::max(smem, narrow_smem_bytes(fl, s.R, s.narrow_wslot));
+        constexpr int S = kWarps, L = kNarrowSpan;
+        s.smem_narrow = narrow_smem_bytes(s.R, s.narrow_wslot);
         const int b_min = ((2 * (2 * s.R + S)) + S - 1) / S * S;       // keep the band prologue below ~50 % extra staging
         int i = s.first_narrow;
         while (i < s.n_north) {
             double c = 0.0; int b = 0;
-            while (i + b < s.n_north && (b < b_min || c < c_max) && b < 256) { c += (double)ring_slots[i + b] * (double)L; b++; }
+            while (i + b < s.n_north && (b < b_min || c < 0.5 * c_max) && b < 512) { c += (double)ring_slots[i + b] * (double)L; b++; }
             b = std::min((b + S - 1) / S * S, s.n_north - i);
             if (s.n_north - (i + b) < b_min / 2) b = s.n_north - i;     // do not leave a tiny tail band
             // the southern mirror band leaves out a ring that is its own mirror (odd n_theta: the equator)
@@ -246,17 +250,20 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
                 uint32_t wcopy = 4;
                 for (int q = 0; q < nb; q++) { c += (double)ring_slots[i + q] * (double)L; wcopy = std::max(wcopy, s.ring_slots[i + q]); }
                 for (int k0 = 0; k0 < n_phi; k0 += L) {
-                    tmp.push_back(Tmp{Item{i, k0, (int16_t)fl, (int16_t)kNarrow, hemi ? -nb : nb, (int32_t)wcopy}, c + 4000.0});
+                    tmp_narrow.push_back(Tmp{Item{i, k0, (int16_t)0, (int16_t)kNarrow, hemi ? -nb : nb, (int32_t)wcopy}, c + 4000.0});
                     for (int q = 0; q < nb; q++) s.fma_slots += ring_slots[i + q] * (unsigned long long)L;
                 }
             }
             i += b;
         }
     }
-    s.smem_bytes = smem;
-    std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; });
-    s.items.reserve(tmp.size());
-    for (auto& t : tmp) s.items.push_back(t.it);
+    auto by_cost = [](const Tmp& a, const Tmp& b) { return a.cost > b.cost; };
+    std::stable_sort(tmp_wide.begin(), tmp_wide.end(), by_cost);
+    std::stable_sort(tmp_narrow.begin(), tmp_narrow.end(), by_cost);
+    s.items.reserve(tmp_wide.size() + tmp_narrow.size());
+    for (auto& t : tmp_wide) s.items.push_back(t.it);
+    s.n_wide_items = (int)s.items.size();
+    for (auto& t : tmp_narrow) s.items.push_back(t.it);
     return validate_schedule(s, nullptr) == 0 ? 0 : 5;
 }
 
@@ -281,15 +288,15 @@ int validate_schedule(const Schedule& s, std::string* why) {
     if (s.s2.size() != (size_t)n_phi / 2 + 1) return fail(5, "s2 size", (long long)s.s2.size(), n_phi);
     if (s.ring_w_off.size() != (size_t)s.n_north || s.ring_slots.size() != (size_t)s.n_north) return fail(6, "ring tables", 0, 0);
     if (s.weight_slots > 0xFFFFFFF0ull) return fail(7, "weight buffer over 2^32 floats", (long long)s.weight_slots, 0);
-    if (s.smem_bytes > (size_t)kSmemBudget) return fail(8, "shared memory over budget", (long long)s.smem_bytes, kSmemBudget);
+    if (s.smem_wide > (size_t)kSmemBudget || s.smem_narrow > (size_t)kSmemBudget) return fail(8, "shared memory over budget", (long long)s.smem_wide, (long long)s.smem_narrow);
+    if (s.n_wide_items < 0 || s.n_wide_items > (int)s.items.size()) return fail(8, "n_wide_items", s.n_wide_items, (long long)s.items.size());
     const long long wtot = (long long)s.weight_slots;
     const bool have_narrow = s.first_narrow < s.n_north;
     if (have_narrow) {
-        if (s.narrow_f_log2 < 0 || s.narrow_f_log2 > 3) return fail(9, "narrow_f_log2", s.narrow_f_log2, 0);
         if (s.narrow_wslot < 4 || s.narrow_wslot % 4 != 0 || s.narrow_w_base % 4 != 0) return fail(10, "narrow weight stride", s.narrow_wslot, s.narrow_w_base);
-        if (narrow_smem_bytes(s.narrow_f_log2, s.R, s.narrow_wslot) > s.smem_bytes) return fail(11, "narrow shared memory", 0, 0);
+        if (narrow_smem_bytes(s.R, s.narrow_wslot) > s.smem_narrow) return fail(11, "narrow shared memory", (long long)s.smem_narrow, 0);
     }
-    if (s.first_narrow > 0 && wide_smem_bytes(s.R) > s.smem_bytes) return fail(12, "wide shared memory", 0, 0);
+    if (s.first_narrow > 0 && wide_smem_bytes(s.R) > s.smem_wide) return fail(12, "wide shared memory", (long long)s.smem_wide, 0);
 
     // ---- pair descriptors (conv_wide: stage source rows and weight ranges; plan_pair_weights) ----------
     unsigned long long stored = 0;
@@ -338,22 +345,25 @@ int validate_schedule(const Schedule& s, std::string* why) {
         gen += (unsigned long long)g.count;
     }
     if (gen != stored) return fail(53, "generator units do not tile the stored taps", (long long)gen, (long long)stored);
-    // ---- work items (k_convolve) and coverage: every output ring x warp tile exactly once -----------------
-    const int tiles = (n_phi + kWarpSpan - 1) / kWarpSpan;
+    // ---- work items (k_convolve_wide / k_convolve_narrow) and coverage: every output ring x 512-pixel tile once ----
+    const int tiles = (n_phi + kNarrowSpan - 1) / kNarrowSpan;
     std::vector<unsigned char> cover((size_t)n_theta * tiles, 0);
-    for (const Item& it : s.items) {
-        if (it.f_log2 < 0 || it.f_log2 > 3) return fail(60, "item f_log2", it.f_log2, 0);
-        const int L = kWarpSpan << it.f_log2;
-        if (it.k0 < 0 || it.k0 >= n_phi || it.k0 % L) return fail(61, "item k0", it.k0, L);
-        const int t0 = it.k0 / kWarpSpan, t1 = std::min(tiles, t0 + (1 << it.f_log2));
+    for (size_t k = 0; k < s.items.size(); k++) {
+        const Item& it = s.items[k];
+        if ((it.kind == kWide) != ((int)k < s.n_wide_items)) return fail(59, "item in the wrong part of the work list", (long long)k, it.kind);
         if (it.kind == kWide) {
+            if (it.f_log2 < 0 || it.f_log2 > 3) return fail(60, "item f_log2", it.f_log2, 0);
+            const int L = kWarpSpan << it.f_log2;
+            if (it.k0 < 0 || it.k0 >= n_phi || it.k0 % L) return fail(61, "item k0", it.k0, L);
             if (it.i0 < 0 || it.i0 >= n_theta) return fail(62, "wide item ring", it.i0, 0);
             const int i_n = 2 * it.i0 >= n_theta ? n_theta - 1 - it.i0 : it.i0;
             if (i_n >= s.first_narrow) return fail(63, "wide item on a narrow ring", it.i0, s.first_narrow);
+            const int t0 = it.k0 / kNarrowSpan, t1 = std::min(tiles, t0 + L / kNarrowSpan);
             for (int t = t0; t < t1; t++) cover[(size_t)it.i0 * tiles + t]++;
         } else if (it.kind == kNarrow) {
             const int nr = it.nrings < 0 ? -it.nrings : it.nrings;
-            if (!have_narrow || it.f_log2 != s.narrow_f_log2) return fail(64, "narrow item tile", it.f_log2, s.narrow_f_log2);
+            if (!have_narrow || it.f_log2 != 0) return fail(64, "narrow item tile", it.f_log2, 0);
+            if (it.k0 < 0 || it.k0 >= n_phi || it.k0 % kNarrowSpan) return fail(61, "item k0", it.k0, kNarrowSpan);
             if (nr < 1 || it.i0 < s.first_narrow || it.i0 + nr > s.n_north) return fail(65, "narrow item band", it.i0, nr);
             if (it.wcopy < 4 || it.wcopy % 4 || it.wcopy > s.narrow_wslot) return fail(66, "narrow item wcopy", it.wcopy, s.narrow_wslot);
             // stage_ring_tables reads wcopy floats of each ring's block
@@ -362,7 +372,7 @@ int validate_schedule(const Schedule& s, std::string* why) {
                 if (s.ring_slots[it.i0 + q] > (unsigned)it.wcopy) return fail(68, "ring block larger than wcopy", it.i0 + q, it.wcopy);
                 const int i_phys = it.nrings < 0 ? n_theta - 1 - (it.i0 + q) : it.i0 + q;
                 if (it.nrings < 0 && 2 * (it.i0 + q) + 1 == n_theta) return fail(69, "self-mirrored ring in a southern band", it.i0 + q, 0);
-                for (int t = t0; t < t1; t++) cover[(size_t)i_phys * tiles + t]++;
+                cover[(size_t)i_phys * tiles + it.k0 / kNarrowSpan]++;
             }
         } else return fail(70, "item kind", it.kind, 0);
     }
@@ -379,10 +389,10 @@ size_t wide_smem_bytes(int R) {
 
 // (2R + 2S) row slots (the S rows of the next pass land in the slots the previous pass freed), two
 // buffers of S ring weight blocks and of S x (2R+1) pair descriptors
-size_t narrow_smem_bytes(int f_log2, int R, int wslot) {
-    const int S = kWarps >> f_log2;
-    return (size_t)(2 * R + 2 * S) * (size_t)narrow_slot_bytes(f_log2) + 2ull * S * (size_t)wslot * 4 +
-           2ull * S * (2 * R + 1) * sizeof(PairDesc);
+size_t narrow_smem_bytes(int R, int wslot) {
+    constexpr int S = kWarps;
+    return (size_t)(2 * R + 2 * S) * (size_t)kNarrowSlotBytes + 2ull * S * (size_t)wslot * 4 +
+           2ull * S * (2 * R + 1) * sizeof(NarrowRun);
 }
 
 }  // namespace arkcos

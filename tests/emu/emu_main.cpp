@@ -126,7 +126,6 @@ int main(int argc, char** argv) {
     Schedule s;
     const int rc = build_schedule(n_theta, n_phi, theta_cut, 148, s);
     if (rc != 0) { std::fprintf(stderr, "build_schedule failed: %d\n", rc); return 2; }
-    if (s.smem_bytes > (size_t)kSmemBudget) { std::fprintf(stderr, "shared memory over budget\n"); return 2; }
     std::vector<float> weights((size_t)s.weight_slots + 4, 0.0f);
     emu::g_global = {{(const unsigned char*)in.data(), (const unsigned char*)(in.data() + in.size())},
                      {(const unsigned char*)weights.data(), (const unsigned char*)(weights.data() + weights.size())},
@@ -164,12 +163,17 @@ int main(int argc, char** argv) {
         if (item_stride > 1 && b % item_stride != 0) continue;
         if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
         (wide ? n_wide : n_narrow)++;
-        emu::run_cta((unsigned)b, 0, kThreads, s.smem_bytes, [&] { k_convolve(c); });
+        ConvParams cc = c;                                     // each kernel is launched on its own part of the work list
+        if (wide) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide(cc); });
+        else {
+            cc.items = c.items + s.n_wide_items;
+            emu::run_cta((unsigned)(b - s.n_wide_items), 0, kThreads, s.smem_narrow, [&] { k_convolve_narrow(cc); });
+        }
     }
     FILE* f = std::fopen(argv[7], "wb");
     if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
     std::fclose(f);
-    std::printf("emu ok: R %d first_narrow %d n_north %d narrow_f_log2 %d items wide %d narrow %d smem %zu weight_slots %llu\n", s.R,
-                s.first_narrow, s.n_north, s.narrow_f_log2, n_wide, n_narrow, s.smem_bytes, (unsigned long long)s.weight_slots);
+    std::printf("emu ok: R %d first_narrow %d n_north %d items wide %d narrow %d smem wide %zu narrow %zu weight_slots %llu\n", s.R,
+                s.first_narrow, s.n_north, n_wide, n_narrow, s.smem_wide, s.smem_narrow, (unsigned long long)s.weight_slots);
     return 0;
 }

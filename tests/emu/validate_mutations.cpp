@@ -49,7 +49,7 @@ int main(int argc, char** argv) {
         {"narrow wcopy beyond the ring stride", [&](Schedule& s) { if (first_narrow_item < 0) return false; s.items[first_narrow_item].wcopy = s.narrow_wslot + 4; return true; }},
         {"narrow wcopy smaller than a ring block", [&](Schedule& s) { if (first_narrow_item < 0) return false; Item& it = s.items[first_narrow_item]; if (s.ring_slots[it.i0] <= 4) return false; it.wcopy = (int)s.ring_slots[it.i0] - 4; return true; }},
         {"narrow wcopy misaligned", [&](Schedule& s) { if (first_narrow_item < 0) return false; s.items[first_narrow_item].wcopy += 2; return true; }},
-        {"narrow item with the wrong tile width", [&](Schedule& s) { if (first_narrow_item < 0) return false; s.items[first_narrow_item].f_log2 = (int16_t)((s.narrow_f_log2 + 1) & 3); return true; }},
+        {"narrow item with the wrong tile width", [&](Schedule& s) { if (first_narrow_item < 0) return false; s.items[first_narrow_item].f_log2 = 1; return true; }},
         {"pair weights beyond the buffer", [&](Schedule& s) { s.pairs[live_pair].w_off = (uint32_t)s.weight_slots; return true; }},
         {"pair weights misaligned", [&](Schedule& s) { s.pairs[live_pair].w_off += 1; return true; }},
         {"pair taps overrun the ring block", [&](Schedule& s) { s.pairs[live_pair].ntaps += 4096; return true; }},
@@ -65,8 +65,10 @@ int main(int argc, char** argv) {
         {"generator unit window", [&](Schedule& s) { s.gen_units[0].half = n_phi / 2; return true; }},
         {"generator unit taps beyond one turn", [&](Schedule& s) { s.gen_units[0].d0 = -n_phi; return true; }},
         {"generator unit dropped", [&](Schedule& s) { s.gen_units.pop_back(); return true; }},
-        {"shared memory too small", [&](Schedule& s) { s.smem_bytes = 1024; return true; }},
-        {"shared memory over budget", [&](Schedule& s) { s.smem_bytes = kSmemBudget + 16; return true; }},
+        {"wide shared memory too small", [&](Schedule& s) { if (s.first_narrow == 0) return false; s.smem_wide = 1024; return true; }},
+        {"narrow shared memory too small", [&](Schedule& s) { if (s.first_narrow >= s.n_north) return false; s.smem_narrow = 1024; return true; }},
+        {"shared memory over budget", [&](Schedule& s) { s.smem_wide = kSmemBudget + 16; return true; }},
+        {"wide / narrow split of the work list", [&](Schedule& s) { if (first_wide < 0 || first_narrow_item < 0) return false; s.n_wide_items -= 1; return true; }},
         {"narrow weight stride misaligned", [&](Schedule& s) { if (s.first_narrow >= s.n_north) return false; s.narrow_wslot += 2; return true; }},
         {"runs table truncated", [&](Schedule& s) { if (s.runs.empty()) return false; s.runs.pop_back(); return true; }},
         {"pairs table truncated", [&](Schedule& s) { s.pairs.pop_back(); return true; }},

@@ -134,7 +134,7 @@ def test_cached_batch_host_and_repeat_calls_are_bit_identical(torch, arkcos):
     stream = torch.cuda.current_stream().cuda_stream
     with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut) as plan, \
             arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=arkcos.PLAN_CACHE_WEIGHTS) as cached:
-        assert plan.info().kernels_per_convolve == 2 and cached.info().kernels_per_convolve == 1
+        assert plan.info().kernels_per_convolve == 3 and cached.info().kernels_per_convolve == 2   # (S2,) S3w, S3
         d_in = torch.from_numpy(maps).cuda()
         single = torch.empty_like(d_in); again = torch.empty_like(d_in); batch = torch.empty_like(d_in)
         c_out = torch.empty_like(d_in)

@@ -119,7 +119,7 @@ def test_work_counts_of_the_baseline_configs(cfg, k, pairs, r):
     assert abs(pe / pairs - 1.0) < 6e-3
     info = p.info()
     assert info.fma_slots >= pe and info.n_items > 0 and info.sm_count == 0
-    assert info.kernels_per_convolve == 2
+    assert info.kernels_per_convolve in (2, 3)          # generator + wide and/or narrow convolution kernel
 
 
 def test_sampled_ring_pair_counts_match_oracle_on_config1():
