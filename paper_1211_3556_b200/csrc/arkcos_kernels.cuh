@@ -397,11 +397,12 @@ __device__ __forceinline__ void narrow_step(float (&a0)[kNarrowP], float (&a1)[k
 // a0[m] + a1[m] += sum_{e < 2 n} wrow[e] * Z[m + 2 k0 + e],  Z = the row from the start of the tile two to the left.
 // zt: shared address of the lane's own tile in the row slot; wq = address of wrow - 8 k0 bytes.
 #pragma nv_diag_suppress 177   // the chain's labels past K = 16 are only fallen into
-__device__ __forceinline__ void narrow_row(float (&a0)[kNarrowP], float (&a1)[kNarrowP], const uint32_t zt, const uint32_t wq, const int k0, int n) {
+__device__ __forceinline__ void narrow_row(float (&a0)[kNarrowP], float (&a1)[kNarrowP], const uint32_t zt, const uint32_t wq, const int k0, const int n) {
     float z[4 * kNarrowRing];
     float w[2][2];
+    const int kend = k0 + n;                                   // the exit test of a step is one compare with an immediate
 #define ARKCOS_NR_CASE(K) case K: narrow_init<K>(z, w, zt, wq); goto nr_step_##K;
-#define ARKCOS_NR_STEP(K) nr_step_##K: narrow_step<K>(a0, a1, z, w, zt, wq); if (--n == 0) goto nr_done;
+#define ARKCOS_NR_STEP(K) nr_step_##K: narrow_step<K>(a0, a1, z, w, zt, wq); if (kend == K + 1) goto nr_done;
     switch (k0) {
         ARKCOS_NR_CASE(0) ARKCOS_NR_CASE(1) ARKCOS_NR_CASE(2) ARKCOS_NR_CASE(3) ARKCOS_NR_CASE(4) ARKCOS_NR_CASE(5)
         ARKCOS_NR_CASE(6) ARKCOS_NR_CASE(7) ARKCOS_NR_CASE(8) ARKCOS_NR_CASE(9) ARKCOS_NR_CASE(10) ARKCOS_NR_CASE(11)
@@ -441,35 +442,39 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     const int lam0 = it.i0, lam_end = it.i0 + nr;
     const int npass = (nr + S - 1) / S;
 
-    // ---- row staging: chunk idx of a row slot = floats [4 idx, 4 idx + 4) from phi = k0 - 32; tile = 4 chunks + pad ----
+    // ---- staging, one warp per row / per ring (all addresses warp uniform except the lane's chunk) ------------
+    // chunk idx of a row slot = floats [4 idx, 4 idx + 4) from phi = k0 - 32, at physical chunk idx + (idx >> 2)
     constexpr int row_chunks = kNarrowSpan / 4 + 2 * (kHaloNarrow / 4);     // own tiles + a halo of 32 floats on either side
-    static_assert(row_chunks <= kThreads, "one cp.async per thread stages a row");
-    const int t_phi = wrap_phi(it.k0 - kHaloNarrow + 4 * (int)threadIdx.x, p.n_phi);
-    const uint32_t t_dst = (uint32_t)((threadIdx.x + (threadIdx.x >> 2)) << 4);
+    const int lane_phi = wrap_phi(it.k0 - kHaloNarrow + 4 * lane, p.n_phi), phi_step = 128 % p.n_phi;
+    const uint32_t lane_dst = (uint32_t)((lane + (lane >> 2)) << 4);
     auto stage_row = [&](const int lam_j) {
         if (lam_j < 0 || lam_j >= p.n_theta) return;          // beyond the pole: no ring pair uses it
-        if ((int)threadIdx.x >= row_chunks) return;
         const float* row = in + (size_t)(south ? p.n_theta - 1 - lam_j : lam_j) * p.n_phi;
         int sl = lam_j % NS; if (sl < 0) sl += NS;
-        cp_async16(rows + (uint32_t)(sl * slot_bytes) + t_dst, row + t_phi);
-    };
-    // weights and run descriptors of the S rings of a pass -> buffer b (no dependent global loads:
-    // both live at computable addresses)
-    const int n4 = it.wcopy >> 2;
-    auto stage_ring_tables = [&](const int pass, const int b) {
-        for (int rs = 0; rs < S; rs++) {
-            const int lam = lam0 + pass * S + rs;
-            if (lam >= lam_end) break;
-            const NarrowRun* psrc = p.runs + (size_t)(lam - p.first_narrow) * W;
-            const uint32_t pdst = pdbuf_addr + (uint32_t)(((b * S + rs) * W) * sizeof(NarrowRun));
-            for (int q = threadIdx.x; q < W; q += kThreads) cp_async16(pdst + 16 * q, psrc + q);
-            const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
-            const uint32_t dst = wbuf_addr + (uint32_t)(((b * S + rs) * p.wslot) * 4);
-            for (int q = threadIdx.x; q < n4; q += kThreads) cp_async16(dst + 16 * q, src + 4 * q);
+        uint32_t dst = rows + (uint32_t)(sl * slot_bytes) + lane_dst;
+        int phi = lane_phi;
+#pragma unroll
+        for (int idx = lane; idx < row_chunks; idx += 32) {
+            cp_async16(dst, row + phi);
+            dst += 40 * 16;                                   // 32 chunks + their 8 pad chunks
+            phi += phi_step;
+            if (phi >= p.n_phi) phi -= p.n_phi;
         }
     };
-    for (int lam_j = lam0 - p.R; lam_j < lam0 + S + p.R; lam_j++) stage_row(lam_j);
-    stage_ring_tables(0, 0);
+    // weights and run descriptors of ring lam -> buffer slot tb (no dependent global loads: both live at
+    // computable addresses)
+    const int n4 = it.wcopy >> 2;
+    auto stage_ring_tables = [&](const int lam, const int tb) {
+        if (lam >= lam_end) return;
+        const NarrowRun* psrc = p.runs + (size_t)(lam - p.first_narrow) * W;
+        const uint32_t pdst = pdbuf_addr + (uint32_t)((tb * W) * sizeof(NarrowRun));
+        for (int q = lane; q < W; q += 32) cp_async16(pdst + 16 * q, psrc + q);
+        const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
+        const uint32_t dst = wbuf_addr + (uint32_t)((tb * p.wslot) * 4);
+        for (int q = lane; q < n4; q += 32) cp_async16(dst + 16 * q, src + 4 * q);
+    };
+    for (int q = s; q < 2 * p.R + S; q += S) stage_row(lam0 - p.R + q);
+    stage_ring_tables(lam0 + s, s);
 
     const uint32_t lane_tile = (uint32_t)((kHaloNarrow / kNarrowP + lane) * kNarrowTileBytes);
     for (int pass = 0; pass < npass; pass++) {
@@ -477,8 +482,8 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
         cp_async_wait_all();
         __syncthreads();                                      // this pass's rows and tables have landed; pass-1 is done
         if (pass + 1 < npass) {                               // next pass: S new rows into the slots pass-1 freed
-            for (int q = 0; q < S; q++) stage_row(lbase + S + p.R + q);
-            stage_ring_tables(pass + 1, (pass + 1) & 1);
+            stage_row(lbase + S + p.R + s);
+            stage_ring_tables(lbase + S + s, ((pass + 1) & 1) * S + s);
         }
         const int lam = lbase + s;
         if (lam < lam_end) {
