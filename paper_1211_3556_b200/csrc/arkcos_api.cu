@@ -88,7 +88,7 @@ arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
     c.runs = pl->d_runs; c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
-    c.n_theta = s.n_theta; c.n_phi = s.n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
+    c.n_theta = s.n_theta; c.n_phi = s.n_phi; c.R = s.R; c.wslot = s.narrow_wslot; c.wcap = s.narrow_wcap;
     c.map_stride = (long long)s.n_theta * s.n_phi;
     const int n_wide = (pl->flags & ARKCOS_PLAN_ONLY_NARROW) ? 0 : s.n_wide_items;
     const int n_narrow = (pl->flags & ARKCOS_PLAN_ONLY_WIDE) ? 0 : (int)s.items.size() - s.n_wide_items;
@@ -214,7 +214,10 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         if (!cuda_ok(cudaFuncSetAttribute(k_convolve_wide, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
                      "cudaFuncSetAttribute(k_convolve_wide)") ||
             !cuda_ok(cudaFuncSetAttribute(k_convolve_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
-                     "cudaFuncSetAttribute(k_convolve_narrow)")) { st = ARKCOS_ECUDA; break; }
+                     "cudaFuncSetAttribute(k_convolve_narrow)") ||
+            // two NARROW CTAs of up to kSmemTwoPerSm share an SM only with the largest shared-memory carve-out
+            !cuda_ok(cudaFuncSetAttribute(k_convolve_narrow, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared),
+                     "cudaFuncSetAttribute(k_convolve_narrow, carveout)")) { st = ARKCOS_ECUDA; break; }
         size_t tab_bytes = (size_t)n_table * sizeof(double);
         pl->table_in_smem = tab_bytes <= (size_t)kGenSmemMax ? 1 : 0;
         pl->gen_smem = pl->table_in_smem ? tab_bytes : 0;

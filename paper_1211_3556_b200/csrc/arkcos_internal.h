@@ -24,6 +24,7 @@ constexpr int kThreads = 32 * kWarps;
 constexpr int kHaloNarrow = 32;        // narrow rings: every stored tap window lies inside [-32, 32)
 constexpr int kGenUnitTaps = 1024;     // taps per weight-generator work unit (one warp)
 constexpr int kSmemBudget = 220 * 1024;
+constexpr int kSmemTwoPerSm = 113 * 1024; // dynamic shared memory of a CTA when two are to share an SM (228 KB - 2 x 1 KB reserved)
 
 // Shared-memory rows are stored in lane tiles: 8 chunks of 16 bytes (the kLaneP floats one lane owns)
 // followed by one pad chunk, so that the 16-byte / 8-byte loads of the 32 lanes of a warp (lane stride
@@ -117,7 +118,8 @@ struct Schedule {
     int n_wide_items = 0;                   // items[0 .. n_wide_items) are WIDE (kernel k_convolve_wide), the rest NARROW
     std::vector<GenUnit> gen_units;
     int first_narrow = 0;                   // rings [first_narrow, n_north) use the narrow kernel path
-    int narrow_wslot = 0;                   // floats per ring in the narrow weight buffers
+    int narrow_wslot = 0;                   // floats per ring in the GLOBAL narrow weight buffer (uniform stride)
+    int narrow_wcap = 0;                    // floats of the weight area in shared memory (conv_narrow)
     size_t smem_wide = 0, smem_narrow = 0;  // dynamic shared memory of the two convolution kernels
     unsigned long long pair_evals = 0;      // useful FMAs per map
     unsigned long long weights = 0;         // in-support weights, no symmetry reduction
@@ -136,7 +138,7 @@ struct Schedule {
 
 // shared memory of a WIDE item (two private stage buffers per warp), and of the NARROW path
 size_t wide_smem_bytes(int R);
-size_t narrow_smem_bytes(int R, int wslot);
+size_t narrow_smem_bytes(int R, int wcap);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
 int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);

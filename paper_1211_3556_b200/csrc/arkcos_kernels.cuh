@@ -107,7 +107,8 @@ struct ConvParams {
     int n_theta, n_phi, R;
     int first_narrow;        // first northern ring of the narrow class
     uint32_t narrow_w_base;  // its weights start here; one block of wslot floats per narrow ring
-    int wslot;               // floats per ring in the narrow weight buffers
+    int wslot;               // floats per ring in the (global) narrow weight buffer
+    int wcap;                // floats of the weight area in conv_narrow's shared memory
     long long map_stride;    // elements between consecutive maps of a batch
 };
 
@@ -435,10 +436,12 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     const int NS = 2 * p.R + 2 * S;                           // row slots
     constexpr int slot_bytes = kNarrowSlotBytes;
     const uint32_t rows = (uint32_t)__cvta_generic_to_shared(smem);
-    float* wbuf = reinterpret_cast<float*>(smem + (size_t)NS * slot_bytes);               // [2][S][wslot]
-    NarrowRun* pdbuf = reinterpret_cast<NarrowRun*>(wbuf + 2 * (size_t)S * p.wslot);      // [2][S][W]
-    const uint32_t wbuf_addr = (uint32_t)__cvta_generic_to_shared(wbuf);
-    const uint32_t pdbuf_addr = (uint32_t)__cvta_generic_to_shared(pdbuf);
+    // shared memory: row slots | run descriptors [2][S][W] | weight area: [2][S][wcopy] if that fits (the tables of
+    // the next pass are then copied during the current one), else [S][wcopy] (every warp reloads its own ring's
+    // block at the start of a pass; only the polar-most bands of the class, whose blocks are the largest)
+    const uint32_t pdbuf_addr = rows + (uint32_t)(NS * slot_bytes);
+    const uint32_t wbuf_addr = pdbuf_addr + (uint32_t)(2 * S * W * sizeof(NarrowRun));
+    const bool dbl = 2 * S * it.wcopy <= p.wcap;
     const int lam0 = it.i0, lam_end = it.i0 + nr;
     const int npass = (nr + S - 1) / S;
 
@@ -470,28 +473,33 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
         const uint32_t pdst = pdbuf_addr + (uint32_t)((tb * W) * sizeof(NarrowRun));
         for (int q = lane; q < W; q += 32) cp_async16(pdst + 16 * q, psrc + q);
         const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
-        const uint32_t dst = wbuf_addr + (uint32_t)((tb * p.wslot) * 4);
+        const uint32_t dst = wbuf_addr + (uint32_t)((tb * it.wcopy) * 4);
         for (int q = lane; q < n4; q += 32) cp_async16(dst + 16 * q, src + 4 * q);
     };
     for (int q = s; q < 2 * p.R + S; q += S) stage_row(lam0 - p.R + q);
-    stage_ring_tables(lam0 + s, s);
+    if (dbl) stage_ring_tables(lam0 + s, s);
 
     const uint32_t lane_tile = (uint32_t)((kHaloNarrow / kNarrowP + lane) * kNarrowTileBytes);
     for (int pass = 0; pass < npass; pass++) {
         const int lbase = lam0 + pass * S;
         cp_async_wait_all();
         __syncthreads();                                      // this pass's rows and tables have landed; pass-1 is done
+        const int lam = lbase + s;
+        if (!dbl) {                                           // this warp's own tables: nobody else reads buffer s
+            stage_ring_tables(lam, s);
+            cp_async_wait_all();
+            __syncwarp();
+        }
         if (pass + 1 < npass) {                               // next pass: S new rows into the slots pass-1 freed
             stage_row(lbase + S + p.R + s);
-            stage_ring_tables(lbase + S + s, ((pass + 1) & 1) * S + s);
+            if (dbl) stage_ring_tables(lbase + S + s, ((pass + 1) & 1) * S + s);
         }
-        const int lam = lbase + s;
         if (lam < lam_end) {
             float a0[kNarrowP], a1[kNarrowP];
 #pragma unroll
             for (int m = 0; m < kNarrowP; m++) { a0[m] = 0.f; a1[m] = 0.f; }
-            const int tb = (pass & 1) * S + s;
-            const uint32_t wring = wbuf_addr + (uint32_t)(tb * p.wslot * 4);
+            const int tb = dbl ? (pass & 1) * S + s : s;
+            const uint32_t wring = wbuf_addr + (uint32_t)(tb * it.wcopy * 4);
             const uint32_t spd = pdbuf_addr + (uint32_t)(tb * W * sizeof(NarrowRun));
             int slot = (lam - p.R) % NS; if (slot < 0) slot += NS;
             uint32_t zt = rows + (uint32_t)(slot * slot_bytes) + lane_tile;

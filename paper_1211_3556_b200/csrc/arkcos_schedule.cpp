@@ -126,24 +126,45 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             const PairDesc& p = s.pairs[(size_t)i * W + r];
             if (p.half >= 0) narrow_range(p.half, nw_start[(size_t)i * W + r], nw_ntaps[(size_t)i * W + r]);
         }
-    // Band marching keeps 2R + 2 kWarps row slots and two buffers of kWarps ring weight blocks in shared memory.
-    // The weight block of a ring grows towards the pole: shrink the narrow class from its polar end until the
-    // launch fits (for a large ring band, R > ~25, nothing fits and every ring takes the WIDE path).
+    // Band marching keeps 2R + 2 kWarps row slots, the run descriptors and the ring weight blocks of kWarps rings in
+    // shared memory.  Whatever the row slots leave of the launch's shared memory is the weight area, `narrow_wcap`
+    // floats: an item whose rings' blocks fit twice (2 kWarps wcopy <= wcap) double-buffers them across passes,
+    // one whose blocks fit once reloads them at the start of every pass (conv_narrow), a ring whose block does
+    // not fit at all is WIDE.  Two launch sizes are tried: half an SM's shared memory, so that two CTAs (16
+    // warps) share an SM - taken when at least 70 % of the narrow FMA slots can then be double-buffered - or else
+    // one CTA per SM with the full budget.  The weight block of a ring grows towards the pole, so the narrow
+    // class shrinks from its polar end; for a large ring band (R > ~25) nothing fits and every ring is WIDE.
     {
         std::vector<unsigned long long> slots(s.n_north, 0);
-        for (int i = s.first_narrow; i < s.n_north; i++)
+        for (int i = s.first_narrow; i < s.n_north; i++) {
             for (int r = 0; r < W; r++) slots[i] += (unsigned long long)nw_ntaps[(size_t)i * W + r];
-        for (;;) {
+            slots[i] = (slots[i] + 3) & ~3ull;
+        }
+        const long long fixed = (long long)narrow_smem_bytes(s.R, 0);
+        auto wcap_of = [&](long long budget) { return budget > fixed ? (budget - fixed) / 4 / 4 * 4 : 0ll; };
+        auto first_fit = [&](long long wcap, int mult) {           // first ring of the class whose block fits `mult` x kWarps times
+            int fn = s.first_narrow;
+            while (fn < s.n_north && (long long)mult * kWarps * (long long)slots[fn] > wcap) fn++;
+            return fn;
+        };
+        const long long wcap2 = wcap_of(kSmemTwoPerSm), wcap1 = wcap_of(kSmemBudget);
+        unsigned long long all = 0, dbl2 = 0;
+        for (int i = s.first_narrow; i < s.n_north; i++) all += slots[i];
+        for (int i = first_fit(wcap2, 2); i < s.n_north; i++) dbl2 += slots[i];
+        long long wcap = 0;
+        if (all > 0 && (double)dbl2 >= 0.7 * (double)all) { wcap = wcap2; s.smem_narrow = (size_t)kSmemTwoPerSm; }
+        else { wcap = wcap1; s.smem_narrow = (size_t)kSmemBudget; }
+        s.first_narrow = first_fit(wcap, 1);
+        if (s.first_narrow >= s.n_north) { s.first_narrow = s.n_north; s.narrow_wslot = 0; s.narrow_wcap = 0; s.smem_narrow = 0; }
+        else {
             unsigned long long wslot = 0;
             for (int i = s.first_narrow; i < s.n_north; i++) wslot = std::max(wslot, slots[i]);
-            s.narrow_wslot = (int)((wslot + 3) & ~3ull);
-            if (s.first_narrow >= s.n_north || narrow_smem_bytes(s.R, s.narrow_wslot) <= (size_t)kSmemBudget) break;
-            // drop the rings whose block is the largest (the polar end), at least one ring
-            int fn = s.first_narrow + 1;
-            while (fn < s.n_north && slots[fn] + 16 > wslot) fn++;
-            s.first_narrow = fn;
+            s.narrow_wslot = (int)wslot;
+            // no more shared memory than the largest item needs (double-buffered if it can be)
+            const long long need = std::min<long long>(wcap, 2ll * kWarps * (long long)wslot);
+            s.narrow_wcap = (int)need;
+            s.smem_narrow = (size_t)(fixed + 4 * need);
         }
-        if (s.first_narrow >= s.n_north) { s.first_narrow = s.n_north; s.narrow_wslot = 0; }
     }
 
     // ---- weight layout ------------------------------------------------------------------------------
@@ -233,14 +254,18 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     // Two CTAs share an SM, so a band is cut at half the WIDE items' cost cap.
     if (s.first_narrow < s.n_north) {
         constexpr int S = kWarps, L = kNarrowSpan;
-        s.smem_narrow = narrow_smem_bytes(s.R, s.narrow_wslot);
+        auto doubles = [&](int i) { return 2ll * S * (long long)s.ring_slots[i] <= (long long)s.narrow_wcap; };
         const int b_min = ((2 * (2 * s.R + S)) + S - 1) / S * S;       // keep the band prologue below ~50 % extra staging
         int i = s.first_narrow;
         while (i < s.n_north) {
+            // a band does not straddle the ring from which the weight blocks fit twice (its wcopy is that of its
+            // polar-most ring, and the kernel double-buffers an item iff 2 kWarps wcopy <= wcap)
+            int limit = s.n_north;
+            if (!doubles(i)) { limit = i + 1; while (limit < s.n_north && !doubles(limit)) limit++; }
             double c = 0.0; int b = 0;
-            while (i + b < s.n_north && (b < b_min || c < 0.5 * c_max) && b < 512) { c += (double)ring_slots[i + b] * (double)L; b++; }
-            b = std::min((b + S - 1) / S * S, s.n_north - i);
-            if (s.n_north - (i + b) < b_min / 2) b = s.n_north - i;     // do not leave a tiny tail band
+            while (i + b < limit && (b < b_min || c < 0.5 * c_max) && b < 512) { c += (double)ring_slots[i + b] * (double)L; b++; }
+            b = std::min((b + S - 1) / S * S, limit - i);
+            if (limit - (i + b) < b_min / 2) b = limit - i;             // do not leave a tiny tail band
             // the southern mirror band leaves out a ring that is its own mirror (odd n_theta: the equator)
             const int b_south = (2 * (i + b - 1) + 1 == n_theta) ? b - 1 : b;
             for (int hemi = 0; hemi < 2; hemi++) {
@@ -294,7 +319,7 @@ int validate_schedule(const Schedule& s, std::string* why) {
     const bool have_narrow = s.first_narrow < s.n_north;
     if (have_narrow) {
         if (s.narrow_wslot < 4 || s.narrow_wslot % 4 != 0 || s.narrow_w_base % 4 != 0) return fail(10, "narrow weight stride", s.narrow_wslot, s.narrow_w_base);
-        if (narrow_smem_bytes(s.R, s.narrow_wslot) > s.smem_narrow) return fail(11, "narrow shared memory", (long long)s.smem_narrow, 0);
+        if (s.narrow_wcap < 0 || s.narrow_wcap % 4 || narrow_smem_bytes(s.R, s.narrow_wcap) > s.smem_narrow) return fail(11, "narrow shared memory", (long long)s.smem_narrow, s.narrow_wcap);
     }
     if (s.first_narrow > 0 && wide_smem_bytes(s.R) > s.smem_wide) return fail(12, "wide shared memory", (long long)s.smem_wide, 0);
 
@@ -366,6 +391,8 @@ int validate_schedule(const Schedule& s, std::string* why) {
             if (it.k0 < 0 || it.k0 >= n_phi || it.k0 % kNarrowSpan) return fail(61, "item k0", it.k0, kNarrowSpan);
             if (nr < 1 || it.i0 < s.first_narrow || it.i0 + nr > s.n_north) return fail(65, "narrow item band", it.i0, nr);
             if (it.wcopy < 4 || it.wcopy % 4 || it.wcopy > s.narrow_wslot) return fail(66, "narrow item wcopy", it.wcopy, s.narrow_wslot);
+            // conv_narrow keeps kWarps (single-buffered) or 2 kWarps (double-buffered) blocks of wcopy floats in the weight area
+            if ((long long)kWarps * it.wcopy > (long long)s.narrow_wcap) return fail(66, "narrow item weight blocks beyond the shared weight area", it.wcopy, s.narrow_wcap);
             // stage_ring_tables reads wcopy floats of each ring's block
             if ((long long)s.narrow_w_base + (long long)(it.i0 + nr - 1 - s.first_narrow) * s.narrow_wslot + it.wcopy > wtot) return fail(67, "narrow weight block beyond the buffer", it.i0, nr);
             for (int q = 0; q < nr; q++) {
@@ -388,11 +415,12 @@ size_t wide_smem_bytes(int R) {
 }
 
 // (2R + 2S) row slots (the S rows of the next pass land in the slots the previous pass freed), two
-// buffers of S ring weight blocks and of S x (2R+1) pair descriptors
-size_t narrow_smem_bytes(int R, int wslot) {
+// buffers of S x (2R+1) run descriptors, and a weight area of `wcap` floats
+size_t narrow_smem_bytes(int R, int wcap) {
     constexpr int S = kWarps;
-    return (size_t)(2 * R + 2 * S) * (size_t)kNarrowSlotBytes + 2ull * S * (size_t)wslot * 4 +
-           2ull * S * (2 * R + 1) * sizeof(NarrowRun);
+    // + 16 bytes: the weight prefetch of a chain step reads the 8 bytes after a run's last weights, which for the
+    // last block of a completely filled weight area would otherwise lie beyond the CTA's shared memory
+    return (size_t)(2 * R + 2 * S) * (size_t)kNarrowSlotBytes + 2ull * S * (2 * R + 1) * sizeof(NarrowRun) + 4ull * (size_t)wcap + 16;
 }
 
 }  // namespace arkcos

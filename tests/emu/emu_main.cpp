@@ -151,7 +151,7 @@ int main(int argc, char** argv) {
     ConvParams c;
     c.in = in.data(); c.out = out.data(); c.pairs = s.pairs.data(); c.items = s.items.data(); c.weights = weights.data();
     c.runs = s.runs.data(); c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
-    c.n_theta = n_theta; c.n_phi = n_phi; c.R = s.R; c.wslot = s.narrow_wslot;
+    c.n_theta = n_theta; c.n_phi = n_phi; c.R = s.R; c.wslot = s.narrow_wslot; c.wcap = s.narrow_wcap;
     c.map_stride = (long long)n_pix;
     emu::g_global.push_back({(const unsigned char*)s.runs.data(), (const unsigned char*)(s.runs.data() + s.runs.size())});
     emu::g_gridDim = dim3((unsigned)s.items.size());
@@ -173,6 +173,9 @@ int main(int argc, char** argv) {
     FILE* f = std::fopen(argv[7], "wb");
     if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
     std::fclose(f);
+    int n_single = 0;
+    for (size_t b = (size_t)s.n_wide_items; b < s.items.size(); b++) n_single += 2 * kWarps * s.items[b].wcopy > s.narrow_wcap;
+    std::printf("single-buffered narrow items %d; ", n_single);
     std::printf("emu ok: R %d first_narrow %d n_north %d items wide %d narrow %d smem wide %zu narrow %zu weight_slots %llu\n", s.R,
                 s.first_narrow, s.n_north, n_wide, n_narrow, s.smem_wide, s.smem_narrow, (unsigned long long)s.weight_slots);
     return 0;

@@ -84,6 +84,9 @@ def test_emulated_kernels_match_oracle(emu_bin, tmp_path, n_theta, n_phi, sigma_
     table = gaussian_table(sigma, cut, 1024)
     x32 = np.random.default_rng(1000 + n_theta).standard_normal((n_theta, n_phi)).astype(np.float32)
     got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    if (n_theta, n_phi) == (301, 256):      # this case must exercise the single-buffered weight tables of conv_narrow
+        import re
+        assert int(re.search(r"single-buffered narrow items (\d+)", log).group(1)) > 0, log
     assert not np.isnan(got).any(), "an output was never written or consumed unstaged shared memory\n" + log
     expect = oracle.convolve(x32, table, cut, level=1)
     rms = math.sqrt((expect ** 2).mean())
@@ -107,7 +110,7 @@ def test_emulated_two_phi_tiles_and_oscillating_kernel(emu_bin, tmp_path):
     assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
 
 
-@pytest.mark.parametrize("n_theta,cut_deg,stride,expect_narrow", [(400, 1.3, 5, True), (96, 9.0, 3, False)])
+@pytest.mark.parametrize("n_theta,cut_deg,stride,expect_narrow", [(400, 1.3, 9, True), (64, 9.0, 7, False)])
 def test_emulated_launch_shapes_of_the_timed_configs(emu_bin, tmp_path, n_theta, cut_deg, stride, expect_narrow):
     """n_phi = 8192, the ring length of configs[2] and configs[4]: WIDE items with F = 8 sub-tiles / S = 1, NARROW
     items with the widest tile.  Every `stride`-th work item is run (EMU_ITEM_STRIDE); the outputs of the
@@ -122,7 +125,7 @@ def test_emulated_launch_shapes_of_the_timed_configs(emu_bin, tmp_path, n_theta,
     assert (int(re.search(r"items wide \d+ narrow (\d+)", log).group(1)) > 0) == expect_narrow, log
     written = ~np.isnan(got)
     rings = np.nonzero(written.any(axis=1))[0]
-    assert len(rings) >= 8 and written.mean() > 0.5 / stride, log
+    assert len(rings) >= 6 and written.mean() > 0.4 / stride, log
     pix = np.flatnonzero(written.reshape(-1))
     pix = pix[:: max(1, len(pix) // 60000)]                     # bounded oracle work
     expect = oracle.convolve(x32, table, cut, level=1, pixels=pix)
