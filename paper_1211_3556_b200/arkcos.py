@@ -18,6 +18,7 @@ from . import build as _build
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, EINTERNAL = 0, 1, 2, 3, 4, 5
 PLAN_DEFAULT, PLAN_HOST_ONLY, PLAN_CACHE_WEIGHTS = 0, 1, 2
 PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos_measure.h)
+PLAN_SPECTRAL = 16                           # N2, the phi-spectral ring-pair path (include/arkcos_spectral.h)
 
 _c_plan_p = ctypes.c_void_p
 
@@ -43,7 +44,7 @@ class ArkcosError(RuntimeError):
 
 _lib = None
 
-# every symbol include/arkcos.h and include/arkcos_measure.h declare: (name, restype, argtypes)
+# every symbol include/arkcos.h, arkcos_measure.h and arkcos_spectral.h declare: (name, restype, argtypes)
 SYMBOLS = [
     ("arkcos_plan_create", ctypes.c_int, [ctypes.POINTER(_c_plan_p), ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
                                           ctypes.c_int, ctypes.c_double]),
@@ -67,6 +68,9 @@ SYMBOLS = [
     ("arkcos_measure_convolve", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
                                                ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
     ("arkcos_plan_validate", ctypes.c_int, [_c_plan_p, ctypes.c_char_p, ctypes.c_int]),
+    ("arkcos_spectral_workspace_bytes", ctypes.c_int, [_c_plan_p, ctypes.c_int, ctypes.POINTER(ctypes.c_ulonglong)]),
+    ("arkcos_convolve_spectral", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
+                                                ctypes.c_ulonglong, ctypes.c_void_p]),
     ("arkcos_plan_item", ctypes.c_int, [_c_plan_p, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
 ]
 
@@ -132,6 +136,16 @@ class Plan:
 
     def convolve_host(self, h_in, h_out, stream: int = 0):
         _check(lib().arkcos_convolve_host(self._h, _ptr(h_in), _ptr(h_out), stream), "arkcos_convolve_host")
+
+    def spectral_workspace_bytes(self, n_maps: int = 1) -> int:
+        b = ctypes.c_ulonglong(0)
+        _check(lib().arkcos_spectral_workspace_bytes(self._h, int(n_maps), ctypes.byref(b)), "arkcos_spectral_workspace_bytes")
+        return int(b.value)
+
+    def convolve_spectral(self, d_in, d_out, d_work, n_maps: int = 1, stream: int = 0):
+        """d_work: a device tensor (any dtype) of at least spectral_workspace_bytes(n_maps) bytes, owned by the caller."""
+        _check(lib().arkcos_convolve_spectral(self._h, _ptr(d_in), _ptr(d_out), int(n_maps), d_work.data_ptr(),
+                                              int(d_work.numel() * d_work.element_size()), stream), "arkcos_convolve_spectral")
 
     def reserve_host_io(self):
         _check(lib().arkcos_plan_reserve_host_io(self._h), "arkcos_plan_reserve_host_io")

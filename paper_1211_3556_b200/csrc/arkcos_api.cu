@@ -3,6 +3,7 @@
 // Product code; shares nothing with oracle/.  No CPU fallback: compute entry points need a CUDA device.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -12,8 +13,10 @@
 
 #include "../../include/arkcos.h"
 #include "../../include/arkcos_measure.h"
+#include "../../include/arkcos_spectral.h"
 #include "arkcos_internal.h"
 #include "arkcos_kernels.cuh"
+#include "arkcos_spectral.cuh"
 
 using namespace arkcos;
 
@@ -46,6 +49,9 @@ struct arkcos_plan {
     NarrowRun* d_runs = nullptr;
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging (arkcos_plan_reserve_host_io)
+    // N2, spectral path (ARKCOS_PLAN_SPECTRAL)
+    float* d_wspec = nullptr;         // [n_north][2R+1][n_phi/2+1] What_ij[m] * 2/n
+    float2 *d_tw_h = nullptr, *d_tw_n = nullptr;
     size_t device_bytes = 0;
     size_t gen_smem = 0;
     int gen_grid = 0, table_in_smem = 0;
@@ -54,16 +60,18 @@ struct arkcos_plan {
 namespace {
 
 template <typename T>
-arkcos_status upload(arkcos_plan* pl, T** dst, const std::vector<T>& src) {
+arkcos_status upload(size_t* counter, T** dst, const std::vector<T>& src) {
     size_t bytes = src.size() * sizeof(T);
     if (bytes == 0) bytes = sizeof(T);
     cudaError_t e = cudaMalloc((void**)dst, bytes);
     if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); return ARKCOS_ENOMEM; }
     CU(e);
-    pl->device_bytes += bytes;
+    *counter += bytes;
     if (!src.empty()) CU(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
     return ARKCOS_OK;
 }
+template <typename T>
+arkcos_status upload(arkcos_plan* pl, T** dst, const std::vector<T>& src) { return upload(&pl->device_bytes, dst, src); }
 
 arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
     GenParams g;
@@ -102,6 +110,62 @@ arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d
         CU(cudaGetLastError());
     }
     return ARKCOS_OK;
+}
+
+// N2: the weight spectra What_ij[m] of every northern ring pair, once per plan (FP64 on the device, rounded to FP32)
+arkcos_status build_spectral(arkcos_plan* pl) {
+    const Schedule& s = pl->sched;
+    const int n = s.n_phi, h = n / 2, W = 2 * s.R + 1;
+    const double kPi = 3.14159265358979323846264338327950288;
+    std::vector<SpecPair> sp((size_t)s.n_north * W);
+    for (int i = 0; i < s.n_north; i++)
+        for (int r = 0; r < W; r++) {
+            const int j = i + r - s.R;
+            SpecPair& g = sp[(size_t)i * W + r];
+            g.half = s.pairs[(size_t)i * W + r].half; g.pad_ = 0;
+            const bool live = g.half >= 0 && j >= 0 && j < s.n_theta;
+            g.a = s.a_r[std::abs(r - s.R)]; g.b = live ? s.sin_t[i] * s.sin_t[j] : 0.0; g.area = live ? s.area[j] : 0.0;
+            if (!live) g.half = -1;
+        }
+    std::vector<double> costab(n);
+    for (int k = 0; k < n; k++) costab[k] = std::cos(2.0 * kPi * k / n);
+    std::vector<float2> tw_h(std::max(1, h / 2)), tw_n(h + 1);
+    for (int k = 0; k < h / 2; k++) tw_h[k] = make_float2((float)std::cos(2.0 * kPi * k / h), (float)-std::sin(2.0 * kPi * k / h));
+    for (int m = 0; m <= h; m++) tw_n[m] = make_float2((float)std::cos(2.0 * kPi * m / n), (float)-std::sin(2.0 * kPi * m / n));
+    SpecPair* d_sp = nullptr; double* d_cos = nullptr;
+    arkcos_status st = ARKCOS_OK;
+    do {
+        if ((st = upload(pl, &pl->d_tw_h, tw_h)) != ARKCOS_OK) break;
+        if ((st = upload(pl, &pl->d_tw_n, tw_n)) != ARKCOS_OK) break;
+        size_t tmp_bytes = 0;                                     // temporaries of this function, not plan memory
+        if ((st = upload(&tmp_bytes, &d_sp, sp)) != ARKCOS_OK) break;
+        if ((st = upload(&tmp_bytes, &d_cos, costab)) != ARKCOS_OK) break;
+        const size_t bytes = sp.size() * (size_t)(h + 1) * sizeof(float);
+        cudaError_t e = cudaMalloc((void**)&pl->d_wspec, bytes);
+        if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); st = ARKCOS_ENOMEM; break; }
+        if (!cuda_ok(e, "cudaMalloc(wspec)")) { st = ARKCOS_ECUDA; break; }
+        pl->device_bytes += bytes;
+        SpecWeightParams w;
+        w.pairs = d_sp; w.s2 = pl->d_s2; w.table = pl->d_table; w.costab = d_cos; w.wspec = pl->d_wspec;
+        w.n_pairs = (int)sp.size(); w.n_phi = n; w.n_table = pl->n_table;
+        w.t_scale = (double)(pl->n_table - 1) / s.theta_cut; w.m_split = pl->m_split; w.theta_split = pl->theta_split; w.t_scale2 = 0.0;
+        if (pl->m_split > 0) {
+            w.t_scale = (double)pl->m_split / pl->theta_split;
+            w.t_scale2 = (double)(pl->n_table - 1 - pl->m_split) / (s.theta_cut - pl->theta_split);
+        }
+        const size_t smem = (size_t)(h + 1) * sizeof(double);
+        if (!cuda_ok(cudaFuncSetAttribute(k_spectral_weights, cudaFuncAttributeMaxDynamicSharedMemorySize, (kSpecMaxPhi / 2 + 1) * 8),
+                     "cudaFuncSetAttribute(k_spectral_weights)") ||
+            !cuda_ok(cudaFuncSetAttribute(k_rfft_rings, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpecMaxPhi * 10 + 16),
+                     "cudaFuncSetAttribute(k_rfft_rings)") ||
+            !cuda_ok(cudaFuncSetAttribute(k_spectral_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpecMaxPhi * 10 + 16),
+                     "cudaFuncSetAttribute(k_spectral_apply)")) { st = ARKCOS_ECUDA; break; }
+        const int grid = std::min<int>((int)sp.size(), 8 * std::max(1, pl->sm_count));
+        k_spectral_weights<<<grid, kSpecThreads, smem, 0>>>(w);
+        if (!cuda_ok(cudaGetLastError(), "k_spectral_weights") || !cuda_ok(cudaDeviceSynchronize(), "k_spectral_weights sync")) { st = ARKCOS_ECUDA; break; }
+    } while (0);
+    cudaFree(d_sp); cudaFree(d_cos);
+    return st;
 }
 
 arkcos_status check_io(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps) {
@@ -146,6 +210,7 @@ arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
         cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
+        cudaFree(pl->d_wspec); cudaFree(pl->d_tw_h); cudaFree(pl->d_tw_n);
         (void)cudaGetLastError();
     }
     delete pl;
@@ -165,7 +230,8 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
     if (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))) return ARKCOS_EINVAL;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
-    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_SPECTRAL)) return ARKCOS_EINVAL;
+    if ((flags & ARKCOS_PLAN_SPECTRAL) && (n_phi < 16 || n_phi > kSpecMaxPhi || (n_phi & (n_phi - 1)) != 0)) return ARKCOS_EUNSUPPORTED;
     if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
     arkcos_plan* pl = new (std::nothrow) arkcos_plan();
@@ -226,6 +292,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         const int units = (int)s.gen_units.size(), per_cta = kGenThreads / 32;
         const int want = (units + per_cta - 1) / per_cta;
         pl->gen_grid = want < pl->sm_count ? (want > 0 ? want : 1) : pl->sm_count;
+        if ((flags & ARKCOS_PLAN_SPECTRAL) && (st = build_spectral(pl)) != ARKCOS_OK) break;
         if (flags & ARKCOS_PLAN_CACHE_WEIGHTS) {
             if ((st = launch_generate(pl, 0)) != ARKCOS_OK) break;
             if (!cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) { st = ARKCOS_ECUDA; break; }
@@ -314,6 +381,35 @@ arkcos_status arkcos_convolve_host(arkcos_plan* pl, const float* h_in, float* h_
     if (s != ARKCOS_OK) return s;
     CU(cudaMemcpyAsync(h_out, pl->d_io_out, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_spectral_workspace_bytes(const arkcos_plan* pl, int n_maps, unsigned long long* bytes) {
+    if (!pl || !bytes || n_maps < 1) return ARKCOS_EINVAL;
+    if (!(pl->flags & ARKCOS_PLAN_SPECTRAL)) return ARKCOS_EUNSUPPORTED;
+    *bytes = (unsigned long long)n_maps * pl->sched.n_theta * (pl->sched.n_phi / 2 + 1) * sizeof(float2);
+    return ARKCOS_OK;
+}
+
+arkcos_status arkcos_convolve_spectral(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, void* d_work,
+                                       unsigned long long work_bytes, void* stream) {
+    arkcos_status st = check_io(pl, d_in, d_out, n_maps);
+    if (st != ARKCOS_OK) return st;
+    if (!(pl->flags & ARKCOS_PLAN_SPECTRAL)) return ARKCOS_EUNSUPPORTED;
+    unsigned long long need = 0;
+    (void)arkcos_spectral_workspace_bytes(pl, n_maps, &need);
+    if (!d_work || ((uintptr_t)d_work & 15u) || work_bytes < need || n_maps > 65535) return ARKCOS_EINVAL;
+    const Schedule& s = pl->sched;
+    const int h = s.n_phi / 2;
+    SpecParams p;
+    p.in = d_in; p.out = d_out; p.xspec = reinterpret_cast<float2*>(d_work); p.wspec = pl->d_wspec; p.pairs = pl->d_pairs;
+    p.tw_h = pl->d_tw_h; p.tw_n = pl->d_tw_n; p.n_theta = s.n_theta; p.n_phi = s.n_phi; p.R = s.R;
+    const dim3 grid((unsigned)s.n_theta, (unsigned)n_maps, 1);
+    cudaStream_t cs = (cudaStream_t)stream;
+    k_rfft_rings<<<grid, kSpecThreads, (size_t)(2 * h + h / 2) * sizeof(float2), cs>>>(p);
+    CU(cudaGetLastError());
+    k_spectral_apply<<<grid, kSpecThreads, (size_t)(2 * h + 1 + h / 2) * sizeof(float2), cs>>>(p);
+    CU(cudaGetLastError());
     return ARKCOS_OK;
 }
 

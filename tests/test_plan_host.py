@@ -23,7 +23,7 @@ def host_plan(n_theta, n_phi, cut, n_table=8):
 
 
 def test_library_exports_every_declared_symbol():
-    header = open(os.path.join(ROOT, "include", "arkcos.h")).read() + open(os.path.join(ROOT, "include", "arkcos_measure.h")).read()
+    header = open(os.path.join(ROOT, "include", "arkcos.h")).read() + open(os.path.join(ROOT, "include", "arkcos_measure.h")).read() + open(os.path.join(ROOT, "include", "arkcos_spectral.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
     declared = set(re.findall(r"\b(arkcos_[a-z_]+)\s*\(", header))
     assert len(declared) >= 12
