@@ -172,8 +172,10 @@ def workload_config(w: wl.Workload):
 
 
 def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
-            only: str = "all"):
-    """One step = S2 + S3 over ALL maps of the workload (configs[4]: the batch of 8 through arkcos_convolve_batch)."""
+            only: str = "all", path: str = "direct"):
+    """One step = S2 + S3 over ALL maps of the workload (configs[4]: the batch of 8 through arkcos_convolve_batch).
+    path = "spectral": the N2 cross-check path (arkcos_convolve_spectral) instead; its step has no S2 (the weight
+    spectra are plan-time) and is timed as a whole."""
     import torch
     from paper_1211_3556_b200 import arkcos
 
@@ -186,17 +188,28 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     # --only wide|narrow: the library's measurement hook launches one class of work items only (the
     # output is then incomplete; used for per-class timing and ncu captures, never for the bench line)
     flags = {"all": 0, "wide": arkcos.PLAN_ONLY_WIDE, "narrow": arkcos.PLAN_ONLY_NARROW}[only]
+    spectral = path == "spectral"
+    if spectral:
+        flags |= arkcos.PLAN_SPECTRAL
     plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
     sh = stream.cuda_stream
+    work = torch.empty(plan.spectral_workspace_bytes(n_maps), dtype=torch.uint8, device=dev) if spectral else None
+
+    def step(src, dst):
+        if spectral:
+            plan.convolve_spectral(src, dst, work, n_maps, sh)
+        else:
+            plan.convolve_batch(src, dst, n_maps, sh)
+
     # rotate input buffers when the map would otherwise sit in L2 between steps
     n_rot = 1 if 8 * w.n_pix * n_maps > 126e6 else max(2, int(math.ceil(260e6 / (4 * w.n_pix))))
     d_in = [torch.from_numpy(x32).to(dev) for _ in range(n_rot)]
     d_out = torch.empty_like(d_in[0])
     with torch.cuda.stream(stream):
         for i in range(warmup):
-            plan.convolve_batch(d_in[i % n_rot], d_out, n_maps, sh)
+            step(d_in[i % n_rot], d_out)
     stream.synchronize()
 
     # ---- timed region: K back-to-back steps, CUDA events on the launching stream --------------------
@@ -209,7 +222,7 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     with torch.cuda.stream(stream):
         e0.record(stream)
         for i in range(steps):
-            plan.convolve_batch(d_in[i % n_rot], d_out, n_maps, sh)
+            step(d_in[i % n_rot], d_out)
         e1.record(stream)
     stream.synchronize()
     torch.cuda.synchronize()
@@ -218,13 +231,20 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     # ---- per-kernel device times (CUDA events inside the library, same stream), K more steps --------
     gen_ms, conv_ms = [], []
     for i in range(steps):
-        g, c = plan.measure_convolve(d_in[i % n_rot], d_out, sh, n_maps)
+        if spectral:                                    # both spectral kernels together, events on the launching stream
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                a.record(stream); step(d_in[i % n_rot], d_out); b.record(stream)
+            stream.synchronize()
+            g, c = 0.0, a.elapsed_time(b)
+        else:
+            g, c = plan.measure_convolve(d_in[i % n_rot], d_out, sh, n_maps)
         gen_ms.append(g); conv_ms.append(c)
     clocks = sampler.stop()
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
-    if want_e2e:
+    if want_e2e and not spectral:
         plan.reserve_host_io()
         h_in = torch.from_numpy(x32[0] if n_maps > 1 else x32).pin_memory()
         h_out = torch.empty_like(h_in).pin_memory()
@@ -243,7 +263,7 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
 
     result = {"elapsed_ms": elapsed_ms, "gen_ms": float(np.mean(gen_ms)), "conv_ms": float(np.mean(conv_ms)),
               "conv_ms_min": float(np.min(conv_ms)), "clocks": clocks, "info": info, "e2e": e2e,
-              "hbm_gbs": hbm_gbs, "sm_max_mhz": sm_max_mhz, "peak_src": peak_src, "n_maps": n_maps,
+              "hbm_gbs": hbm_gbs, "sm_max_mhz": sm_max_mhz, "peak_src": peak_src, "n_maps": n_maps, "path": path,
               "device_name": torch.cuda.get_device_name(dev), "sm_count": info.sm_count}
     plan.destroy()
     return result
@@ -291,6 +311,26 @@ def build_line(w, args, res, world, total_ms, total_units, cpu):
     return line
 
 
+def spectral_line(line, w, res):
+    """The N2 path is bound by memory traffic, not by the FP32 ALUs: per map it reads the map, writes and re-reads
+    the ring spectra X_j (2R+1 times, mostly from L2), reads the weight spectra once and writes the result.  The
+    roofline entry is therefore recomputed against HBM with the traffic that MUST cross HBM: map in + out (8 B per
+    pixel), the spectra written once and read at least once (2 x 8 B per mode), and the weight spectra (4 B per
+    ring pair and mode, read once per call and shared by the maps of a batch)."""
+    info = res["info"]
+    n_maps = res["n_maps"]
+    h1 = w.n_phi // 2 + 1
+    w_rows = ((w.n_theta + 1) // 2) * (2 * int(info.ring_halfband) + 1)
+    bytes_alg = n_maps * (8.0 * w.n_pix + 16.0 * w.n_theta * h1) + 4.0 * w_rows * h1
+    ach = bytes_alg / (res["conv_ms"] * 1e-3) / 1e9
+    line["config"]["path"] = "spectral (N2 cross-check path, include/arkcos_spectral.h)"
+    line["kernel_ms"] = {"rfft_rings+spectral_apply": res["conv_ms"]}
+    line["roofline"] = {"bound": "hbm", "achieved": ach, "peak": res["hbm_gbs"], "unit": "GB/s", "frac": ach / res["hbm_gbs"],
+                        "traffic": None, "kernel": "k_rfft_rings + k_spectral_apply", "algorithmic_bytes_per_launch": bytes_alg,
+                        "peak_source": "hbm_gbs, %s MEASURED_PEAKS.json" % res["peak_src"]}
+    line["gpu_launches"] = line["steps"] * 2
+
+
 def cpu_baseline(w: wl.Workload, n_pixels: int):
     pairs, dt, cores = oracle_sample(w, n_pixels, 4242)
     return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "tuned": False,
@@ -310,6 +350,8 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=1 << 17, help="oracle sample per step of --impl reference")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="five-config report + cost-vs-theta_cut curve")
+    ap.add_argument("--path", default="direct", choices=["direct", "spectral"],
+                    help="direct = the product's hot path (S2 + S3); spectral = the N2 cross-check path (arkcos_convolve_spectral)")
     ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
                     help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
                          "prints a per-class line, not the bench line)")
@@ -345,12 +387,14 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False)
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, path=args.path)
     units = float(res["info"].pair_evals) * res["n_maps"] * args.steps
     total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
     if rank == 0:
         cpu = None if (args.no_cpu or world > 1) else cpu_baseline(w, args.cpu_pixels)
         line = build_line(w, args, res, world, total_ms, total_units, cpu)
+        if args.path == "spectral":
+            spectral_line(line, w, res)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -362,13 +406,18 @@ def sweep(args):
     (a*cut^2 + c, and the paper's linear form of Eq. 2.3)."""
     curve = {}
     for w in wl.all_workloads():
-        res = measure(w, max(3, args.steps // 2), 3, None, 0, want_cpu=False, want_e2e=False)
-        a = argparse.Namespace(**vars(args)); a.steps = max(3, args.steps // 2)
-        line = build_line(w, a, res, 1, res["elapsed_ms"], float(res["info"].pair_evals) * res["n_maps"] * a.steps, None)
-        line["report"] = "sweep"
-        print(json.dumps(line), flush=True)
-        key = w.name.split("_cut")[0]
-        curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"] / res["n_maps"]))
+        for path in ("direct", "spectral"):
+            if path == "spectral" and (w.n_phi & (w.n_phi - 1) or w.n_phi < 16):
+                continue
+            res = measure(w, max(3, args.steps // 2), 3, None, 0, want_cpu=False, want_e2e=False, path=path)
+            a = argparse.Namespace(**vars(args)); a.steps = max(3, args.steps // 2)
+            line = build_line(w, a, res, 1, res["elapsed_ms"], float(res["info"].pair_evals) * res["n_maps"] * a.steps, None)
+            if path == "spectral":
+                spectral_line(line, w, res)
+            line["report"] = "sweep"
+            print(json.dumps(line), flush=True)
+            key = w.name.split("_cut")[0] + ("" if path == "direct" else " [spectral path]")
+            curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"] / res["n_maps"]))
     for key, pts in curve.items():
         if len(pts) < 3:
             continue

@@ -132,3 +132,26 @@ def test_emulated_launch_shapes_of_the_timed_configs(emu_bin, tmp_path, n_theta,
     full_rms = math.sqrt((expect ** 2).mean())
     err = got.reshape(-1)[pix] - expect
     assert math.sqrt((err ** 2).mean()) / full_rms <= 1e-6 and float(np.abs(err).max()) / full_rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("n_theta,n_phi,cut_in_dtheta,stride,single", [(320, 640, 12.52, 2, False), (384, 768, 15.17, 3, True)])
+def test_emulated_medium_ring_bands_march(emu_bin, tmp_path, n_theta, n_phi, cut_in_dtheta, stride, single):
+    """R = 12 and R = 15, the ring half bands of configs[3] at 2 x FWHM and configs[4] at 40': the
+    equatorial rings take the band-marching NARROW path (2R + 16 row slots, one CTA per SM), the polar-most band of
+    the R = 15 case with single-buffered weight tables.  A sign-changing kernel; every `stride`-th work item."""
+    import re
+    cut = cut_in_dtheta * math.pi / n_theta
+    th = np.linspace(0.0, cut, 2048)
+    table = np.cos(3.0 * th / cut) * np.exp(-0.5 * (th / (cut / 3.0)) ** 2)
+    x32 = np.random.default_rng(n_theta).standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut, env={"EMU_ITEM_STRIDE": str(stride)})
+    assert int(re.search(r"items wide \d+ narrow (\d+)", log).group(1)) > 0, log
+    assert (int(re.search(r"single-buffered narrow items (\d+)", log).group(1)) > 0) == single, log
+    written = ~np.isnan(got)
+    pix = np.flatnonzero(written.reshape(-1))
+    assert written.mean() > 0.2
+    pix = pix[:: max(1, len(pix) // 40000)]
+    expect = oracle.convolve(x32, table, cut, level=1, pixels=pix)
+    rms = math.sqrt((expect ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
