@@ -49,6 +49,12 @@ struct arkcos_plan {
     NarrowRun* d_runs = nullptr;
     float* d_weights = nullptr;
     float *d_io_in = nullptr, *d_io_out = nullptr;   // arkcos_convolve_host staging (arkcos_plan_reserve_host_io)
+    // arkcos_convolve_host pipeline (arkcos_plan_reserve_host_io)
+    Pipeline pipe;
+    Item* d_pipe_items = nullptr;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    std::vector<cudaEvent_t> ev_h2d, ev_comp;
+    cudaEvent_t ev_fork = nullptr;
     // N2, spectral path (ARKCOS_PLAN_SPECTRAL)
     float* d_wspec = nullptr;         // [n_north][2R+1][n_phi/2+1] What_ij[m] * 2/n
     float2 *d_tw_h = nullptr, *d_tw_n = nullptr;
@@ -89,27 +95,40 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
     return ARKCOS_OK;
 }
 
-// S3 / S3w: the WIDE items (k_convolve_wide, one CTA per SM) and the NARROW items (k_convolve_narrow, two CTAs per
-// SM) of the plan, back to back on the caller's stream.  The two kernels write disjoint output rings.
-arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
+ConvParams conv_params(const arkcos_plan* pl, const float* d_in, float* d_out) {
     const Schedule& s = pl->sched;
     ConvParams c;
     c.in = d_in; c.out = d_out; c.pairs = pl->d_pairs; c.items = pl->d_items; c.weights = pl->d_weights;
     c.runs = pl->d_runs; c.first_narrow = s.first_narrow; c.narrow_w_base = s.narrow_w_base;
     c.n_theta = s.n_theta; c.n_phi = s.n_phi; c.R = s.R; c.wslot = s.narrow_wslot; c.wcap = s.narrow_wcap;
     c.map_stride = (long long)s.n_theta * s.n_phi;
-    const int n_wide = (pl->flags & ARKCOS_PLAN_ONLY_NARROW) ? 0 : s.n_wide_items;
-    const int n_narrow = (pl->flags & ARKCOS_PLAN_ONLY_WIDE) ? 0 : (int)s.items.size() - s.n_wide_items;
+    return c;
+}
+
+// n_wide WIDE items at `wide`, n_narrow NARROW items at `narrow` (device pointers), back to back on `st`
+arkcos_status launch_items(const arkcos_plan* pl, ConvParams c, const Item* wide, int n_wide, const Item* narrow, int n_narrow,
+                           int n_maps, cudaStream_t st) {
+    if (pl->flags & ARKCOS_PLAN_ONLY_NARROW) n_wide = 0;
+    if (pl->flags & ARKCOS_PLAN_ONLY_WIDE) n_narrow = 0;
     if (n_wide > 0) {
-        k_convolve_wide<<<dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, s.smem_wide, st>>>(c);
+        c.items = wide;
+        k_convolve_wide<<<dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st>>>(c);
         CU(cudaGetLastError());
     }
     if (n_narrow > 0) {
-        c.items = pl->d_items + s.n_wide_items;
-        k_convolve_narrow<<<dim3((unsigned)n_narrow, (unsigned)n_maps, 1), kThreads, s.smem_narrow, st>>>(c);
+        c.items = narrow;
+        k_convolve_narrow<<<dim3((unsigned)n_narrow, (unsigned)n_maps, 1), kThreads, pl->sched.smem_narrow, st>>>(c);
         CU(cudaGetLastError());
     }
     return ARKCOS_OK;
+}
+
+// S3 / S3w: the WIDE items (k_convolve_wide, one CTA per SM) and the NARROW items (k_convolve_narrow, two CTAs per
+// SM) of the plan, back to back on the caller's stream.  The two kernels write disjoint output rings.
+arkcos_status launch_convolve(const arkcos_plan* pl, const float* d_in, float* d_out, int n_maps, cudaStream_t st) {
+    const Schedule& s = pl->sched;
+    return launch_items(pl, conv_params(pl, d_in, d_out), pl->d_items, s.n_wide_items, pl->d_items + s.n_wide_items,
+                        (int)s.items.size() - s.n_wide_items, n_maps, st);
 }
 
 // N2: the weight spectra What_ij[m] of every northern ring pair, once per plan (FP64 on the device, rounded to FP32)
@@ -210,7 +229,12 @@ arkcos_status arkcos_plan_destroy(arkcos_plan* pl) {
     if (!(pl->flags & ARKCOS_PLAN_HOST_ONLY)) {
         cudaFree(pl->d_pairs); cudaFree(pl->d_items); cudaFree(pl->d_units); cudaFree(pl->d_runs); cudaFree(pl->d_s2); cudaFree(pl->d_table);
         cudaFree(pl->d_weights); cudaFree(pl->d_io_in); cudaFree(pl->d_io_out);
-        cudaFree(pl->d_wspec); cudaFree(pl->d_tw_h); cudaFree(pl->d_tw_n);
+        cudaFree(pl->d_wspec); cudaFree(pl->d_tw_h); cudaFree(pl->d_tw_n); cudaFree(pl->d_pipe_items);
+        for (auto& e : pl->ev_h2d) if (e) cudaEventDestroy(e);
+        for (auto& e : pl->ev_comp) if (e) cudaEventDestroy(e);
+        if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
+        if (pl->s_h2d) cudaStreamDestroy(pl->s_h2d);
+        if (pl->s_d2h) cudaStreamDestroy(pl->s_d2h);
         (void)cudaGetLastError();
     }
     delete pl;
@@ -357,6 +381,10 @@ arkcos_status arkcos_plan_reserve_host_io(arkcos_plan* pl) {
     if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
     if (pl->d_io_in) return ARKCOS_OK;
     const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
+    // chunks of about 8 MB: long enough for the copy engines, short enough that compute and the copy back start early
+    const int n_chunks = (int)std::max<size_t>(1, std::min<size_t>(16, bytes / (8u << 20)));
+    arkcos_status st = ARKCOS_OK;
+    try { build_pipeline(pl->sched, n_chunks, pl->pipe); } catch (const std::bad_alloc&) { return ARKCOS_ENOMEM; }
     cudaError_t e = cudaMalloc((void**)&pl->d_io_in, bytes);
     if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d_io_out, bytes);
     if (e != cudaSuccess) {
@@ -365,21 +393,54 @@ arkcos_status arkcos_plan_reserve_host_io(arkcos_plan* pl) {
         CU(e);
     }
     pl->device_bytes += 2 * bytes;
+    if ((st = upload(pl, &pl->d_pipe_items, pl->pipe.items)) != ARKCOS_OK) return st;
+    CU(cudaStreamCreateWithFlags(&pl->s_h2d, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&pl->s_d2h, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+    pl->ev_h2d.assign(pl->pipe.n_chunks, nullptr); pl->ev_comp.assign(pl->pipe.n_chunks, nullptr);
+    for (auto& ev : pl->ev_h2d) CU(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    for (auto& ev : pl->ev_comp) CU(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    CU(cudaDeviceSynchronize());                                  // the item upload has landed
     return ARKCOS_OK;
 }
 
+// HOST map in, HOST map out, as a pipeline over bands of rings (Pipeline, arkcos_internal.h): the copy of chunk
+// c + 1 to the device, the convolution of the items whose last input ring lies in chunk c, and the copy back of the
+// chunks those items completed run concurrently on three streams.  The work items, their kernels and therefore
+// the result are those of arkcos_convolve.
 arkcos_status arkcos_convolve_host(arkcos_plan* pl, const float* h_in, float* h_out, void* stream) {
     if (!pl || !h_in || !h_out) return ARKCOS_EINVAL;
     if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
     arkcos_status s = arkcos_plan_reserve_host_io(pl);           // no-op once reserved
     if (s != ARKCOS_OK) return s;
     if ((s = check_io(pl, pl->d_io_in, pl->d_io_out, 1)) != ARKCOS_OK) return s;
-    const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
+    const Pipeline& pp = pl->pipe;
+    const size_t row = (size_t)pl->sched.n_phi;
     cudaStream_t st = (cudaStream_t)stream;
-    CU(cudaMemcpyAsync(pl->d_io_in, h_in, bytes, cudaMemcpyHostToDevice, st));
-    s = run(pl, pl->d_io_in, pl->d_io_out, 1, st);
-    if (s != ARKCOS_OK) return s;
-    CU(cudaMemcpyAsync(h_out, pl->d_io_out, bytes, cudaMemcpyDeviceToHost, st));
+    // the copy streams start after whatever the caller has queued on `stream`
+    CU(cudaEventRecord(pl->ev_fork, st));
+    CU(cudaStreamWaitEvent(pl->s_h2d, pl->ev_fork, 0));
+    CU(cudaStreamWaitEvent(pl->s_d2h, pl->ev_fork, 0));
+    if (!(pl->flags & ARKCOS_PLAN_CACHE_WEIGHTS) && (s = launch_generate(pl, st)) != ARKCOS_OK) return s;
+    const ConvParams c = conv_params(pl, pl->d_io_in, pl->d_io_out);
+    for (int g = 0; g < pp.n_chunks; g++) {
+        const size_t lo = (size_t)pp.chunk_lo[g] * row, n = (size_t)(pp.chunk_lo[g + 1] - pp.chunk_lo[g]) * row;
+        CU(cudaMemcpyAsync(pl->d_io_in + lo, h_in + lo, n * sizeof(float), cudaMemcpyHostToDevice, pl->s_h2d));
+        CU(cudaEventRecord(pl->ev_h2d[g], pl->s_h2d));
+        CU(cudaStreamWaitEvent(st, pl->ev_h2d[g], 0));
+        s = launch_items(pl, c, pl->d_pipe_items + pp.wide_begin[g], pp.narrow_begin[g] - pp.wide_begin[g],
+                         pl->d_pipe_items + pp.narrow_begin[g], pp.wide_begin[g + 1] - pp.narrow_begin[g], 1, st);
+        if (s != ARKCOS_OK) return s;
+        CU(cudaEventRecord(pl->ev_comp[g], st));
+        bool waited = false;
+        for (int ch = 0; ch < pp.n_chunks; ch++) {
+            if (pp.ready_group[ch] != g) continue;
+            if (!waited) { CU(cudaStreamWaitEvent(pl->s_d2h, pl->ev_comp[g], 0)); waited = true; }
+            const size_t clo = (size_t)pp.chunk_lo[ch] * row, cn = (size_t)(pp.chunk_lo[ch + 1] - pp.chunk_lo[ch]) * row;
+            CU(cudaMemcpyAsync(h_out + clo, pl->d_io_out + clo, cn * sizeof(float), cudaMemcpyDeviceToHost, pl->s_d2h));
+        }
+    }
+    CU(cudaStreamSynchronize(pl->s_d2h));
     CU(cudaStreamSynchronize(st));
     return ARKCOS_OK;
 }

@@ -136,6 +136,22 @@ struct Schedule {
     }
 };
 
+// Host <-> device pipeline of arkcos_convolve_host: the map is cut into `n_chunks` bands of rings; chunk c is copied to
+// the device, then the work items whose LAST input ring lies in chunk c (their "group") are launched, and a chunk's
+// output rings are copied back as soon as every item that writes into it has been launched.  Same items, same
+// arithmetic as one arkcos_convolve: only the launches are grouped, so the result is bit-identical.
+struct Pipeline {
+    int n_chunks = 0;
+    std::vector<int> chunk_lo;              // [n_chunks + 1] first ring of each chunk; chunk_lo[n_chunks] = n_theta
+    std::vector<Item> items;                // the schedule's items ordered by (group, class, cost)
+    std::vector<int> wide_begin;            // [n_chunks + 1] items[wide_begin[g] .. narrow_begin[g]) = WIDE items of group g
+    std::vector<int> narrow_begin;          // [n_chunks + 1] items[narrow_begin[g] .. wide_begin[g + 1]) = NARROW items of group g
+    std::vector<int> ready_group;           // [n_chunks] chunk c's output is complete once groups <= ready_group[c] have run
+};
+// physical output rings [lo, hi] of a work item
+void item_output_rings(const Schedule& s, const Item& it, int& lo, int& hi);
+void build_pipeline(const Schedule& s, int n_chunks, Pipeline& out);
+
 // shared memory of a WIDE item (two private stage buffers per warp), and of the NARROW path
 size_t wide_smem_bytes(int R);
 size_t narrow_smem_bytes(int R, int wcap);

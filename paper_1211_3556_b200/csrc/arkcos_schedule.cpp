@@ -408,6 +408,43 @@ int validate_schedule(const Schedule& s, std::string* why) {
     return 0;
 }
 
+void item_output_rings(const Schedule& s, const Item& it, int& lo, int& hi) {
+    if (it.kind == kWide) { lo = hi = it.i0; return; }
+    const int nr = it.nrings < 0 ? -it.nrings : it.nrings;
+    if (it.nrings < 0) { lo = s.n_theta - it.i0 - nr; hi = s.n_theta - 1 - it.i0; }
+    else { lo = it.i0; hi = it.i0 + nr - 1; }
+}
+
+void build_pipeline(const Schedule& s, int n_chunks, Pipeline& p) {
+    p = Pipeline();
+    n_chunks = std::max(1, std::min(n_chunks, s.n_theta));
+    p.n_chunks = n_chunks;
+    p.chunk_lo.resize(n_chunks + 1);
+    for (int c = 0; c <= n_chunks; c++) p.chunk_lo[c] = (int)((long long)s.n_theta * c / n_chunks);
+    auto chunk_of = [&](int ring) { return (int)(std::upper_bound(p.chunk_lo.begin(), p.chunk_lo.end(), ring) - p.chunk_lo.begin()) - 1; };
+    struct Tmp { int group, kind; size_t order; };
+    std::vector<Tmp> key(s.items.size());
+    p.ready_group.assign(n_chunks, 0);
+    for (size_t k = 0; k < s.items.size(); k++) {
+        int lo, hi;
+        item_output_rings(s, s.items[k], lo, hi);
+        const int g = chunk_of(std::min(s.n_theta - 1, hi + s.R));   // the last input ring the item reads
+        key[k] = Tmp{g, s.items[k].kind, k};
+        for (int c = chunk_of(lo); c <= chunk_of(hi); c++) p.ready_group[c] = std::max(p.ready_group[c], g);
+    }
+    std::stable_sort(key.begin(), key.end(), [](const Tmp& a, const Tmp& b) { return a.group != b.group ? a.group < b.group : a.kind < b.kind; });
+    p.items.reserve(key.size());
+    p.wide_begin.assign(n_chunks + 1, 0); p.narrow_begin.assign(n_chunks + 1, 0);
+    size_t k = 0;
+    for (int g = 0; g < n_chunks; g++) {
+        p.wide_begin[g] = (int)p.items.size();
+        while (k < key.size() && key[k].group == g && key[k].kind == kWide) p.items.push_back(s.items[key[k++].order]);
+        p.narrow_begin[g] = (int)p.items.size();
+        while (k < key.size() && key[k].group == g) p.items.push_back(s.items[key[k++].order]);
+    }
+    p.wide_begin[n_chunks] = p.narrow_begin[n_chunks] = (int)p.items.size();
+}
+
 size_t wide_smem_bytes(int R) {
     const size_t stage = (size_t)kWarps * 2 * kWideStageBytes + (size_t)(2 * R + 1) * sizeof(PairDesc);
     const size_t red = (size_t)kWarps * kWarpSpan * 4;

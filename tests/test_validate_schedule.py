@@ -54,3 +54,23 @@ def test_validator_rejects_every_single_field_corruption(mutations_bin, n_theta,
     res = subprocess.run([mutations_bin, str(n_theta), str(n_phi), repr(cut)], capture_output=True, text=True, timeout=300)
     assert res.returncode == 0, res.stdout + res.stderr
     assert "mutations rejected" in res.stdout
+
+
+@pytest.fixture(scope="module")
+def pipeline_bin(tmp_path_factory):
+    out = str(tmp_path_factory.mktemp("pc") / "pipeline_check")
+    cmd = ["g++", "-std=c++17", "-O1", "-g", "-fsanitize=address", "-I", CSRC, os.path.join(EMU_DIR, "pipeline_check.cpp"),
+           os.path.join(CSRC, "arkcos_schedule.cpp"), "-o", out]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr[-3000:]
+    return out
+
+
+@pytest.mark.parametrize("n_theta,n_phi,cut", [(64, 128, math.radians(9.0)), (4096, 8192, 15.0 * wl.ARCMIN), (2048, 4096, 66.0 * wl.ARCMIN),
+                                               (9, 16, math.radians(50.0)), (301, 256, math.radians(3.69)), (4096, 8192, 40.0 * wl.ARCMIN)])
+def test_host_pipeline_schedule_invariants(pipeline_bin, n_theta, n_phi, cut):
+    """arkcos_convolve_host overlaps the copy in, the convolution and the copy back over bands of rings (VERDICT r1
+    item 8).  tests/emu/pipeline_check.cpp: every item runs once, only after its input rings are on the device, and
+    a band is copied back only after every item that writes into it has been launched."""
+    res = subprocess.run([pipeline_bin, str(n_theta), str(n_phi), repr(cut)], capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
