@@ -121,3 +121,64 @@ def test_gpu_biased_table_weights_and_map():
     expect = oracle.convolve(x32, table, CUT, level=1, m_split=M_SPLIT, theta_split=T_SPLIT)
     rms = math.sqrt((expect ** 2).mean())
     assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5
+
+
+# ------------------------------------------------------------------ the paper's own regime (second half) ---
+def paper_regime_table(w):
+    """The oscillatory residual kernel of configs[4] on the paper's two-zone nodes: half the nodes in the first 1/16
+    of the support."""
+    m_split, t_split = (w.n_table - 1) // 2, w.theta_cut / 16.0
+    nodes = wl.biased_nodes(w.theta_cut, w.n_table, m_split, t_split)
+    return wl.residual_profile(nodes, w.sigma, w.l_band), m_split, t_split
+
+
+def test_emulated_large_ring_band_with_the_papers_table(emu_bin, tmp_path):  # noqa: F811
+    """A small-scale analogue of the paper's regime (theta_cut = 240' on nside 2048, R = 91): R = 23 ring
+    half band (every ring WIDE, 47 input rows per output ring), an oscillatory kernel on the two-zone table."""
+    n_theta, n_phi = 120, 256
+    cut = 23.4 * math.pi / n_theta
+    m_split, t_split = 128, cut / 16.0
+    nodes = wl.biased_nodes(cut, 257, m_split, t_split)
+    table = np.cos(9.0 * nodes / cut) * np.exp(-0.5 * (nodes / (0.35 * cut)) ** 2)
+    x32 = np.random.default_rng(91).standard_normal((n_theta, n_phi)).astype(np.float32)
+    os.environ["EMU_M_SPLIT"], os.environ["EMU_THETA_SPLIT"], os.environ["EMU_ITEM_STRIDE"] = str(m_split), repr(t_split), "3"
+    try:
+        got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    finally:
+        del os.environ["EMU_M_SPLIT"], os.environ["EMU_THETA_SPLIT"], os.environ["EMU_ITEM_STRIDE"]
+    assert "R 23" in log, log
+    written = ~np.isnan(got)
+    pix = np.flatnonzero(written.reshape(-1))
+    assert written.mean() > 0.25
+    expect = oracle.convolve(x32, table, cut, level=1, pixels=pix, m_split=m_split, theta_split=t_split)
+    rms = math.sqrt((expect ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.gpu
+def test_gpu_paper_regime_240_arcmin_sampled():
+    """theta_cut = 240' on 4096 x 8192 (R = 91; 2.9e12 kernel-pixel evaluations), the residual kernel on the paper's
+    two-zone table; sampled output pixels (poles, equator, seeded random) against the oracle."""
+    import torch
+    from paper_1211_3556_b200 import arkcos
+    assert torch.cuda.is_available()
+    w = wl.paper_regime_workload()
+    table, m_split, t_split = paper_regime_table(w)
+    x32 = w.map_f32()
+    with arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, m_split=m_split, theta_split=t_split) as plan:
+        assert plan.work()[2] == 91
+        d_in = torch.from_numpy(x32).cuda()
+        d_out = torch.full_like(d_in, float("nan"))
+        plan.convolve(d_in, d_out, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy()
+    assert np.isfinite(got).all()
+    rng = np.random.default_rng(240)
+    ks = [0, 1, 31, 32, 1023, 1024, 1025, 4095, 4096, 8191]
+    rings = [0, 1, 90, 91, 92, 183, 184, 1000, 2047, 2048, 4095 - 91, 4095]
+    pix = np.array(sorted({i * w.n_phi + k for i in rings for k in ks} | {int(p) for p in rng.integers(0, w.n_pix, 300)}), dtype=np.int64)
+    expect = oracle.convolve(x32, table, w.theta_cut, level=1, pixels=pix, m_split=m_split, theta_split=t_split)
+    scale = math.sqrt((got.astype(np.float64) ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / scale <= 1e-6 and float(np.abs(err).max()) / scale <= 1e-5
