@@ -289,7 +289,7 @@ def build_line(w, args, res, world, total_ms, total_units, cpu):
         "roofline": {
             "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
             "frac": achieved_tflops / peak_tflops, "traffic": traffic, "traffic_source": traffic_src,
-            "kernel": "k_convolve", "flops_per_launch": 2.0 * pair_evals,
+            "kernel": "k_convolve_wide + k_convolve_narrow (the two launches of step S3, timed together)", "flops_per_launch": 2.0 * pair_evals,
             "peak_source": "%d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json)" % (
                 res["sm_count"], res["sm_max_mhz"], res["peak_src"]),
             "issued_lane_frac": float(info.fma_slots) * n_maps / (res["conv_ms"] * 1e-3) / (peak_tflops * 1e12 / 2.0),

@@ -344,6 +344,7 @@ def test_one_plan_on_two_streams_concurrently(torch, arkcos):
         torch.cuda.synchronize()
         streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         outs = [[torch.full_like(d_in[0], float("nan")) for _ in range(6)] for _ in range(2)]
+        torch.cuda.synchronize()        # the NaN fills run on the default stream, which the side streams do not wait for
         for rep in range(6):
             for m in range(2):
                 plan.convolve(d_in[m], outs[m][rep], streams[m].cuda_stream)
