@@ -155,3 +155,21 @@ def test_emulated_medium_ring_bands_march(emu_bin, tmp_path, n_theta, n_phi, cut
     rms = math.sqrt((expect ** 2).mean())
     err = got.reshape(-1)[pix] - expect
     assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("n_theta,n_phi,cut_deg", [
+    (1, 4, 10.0), (1, 4, 180.0), (2, 8, 95.0), (3, 8, 61.0), (7, 12, 100.0), (9, 16, 50.0), (10, 20, 180.0),
+    (16, 32, 7.0), (16, 32, 3.0), (33, 64, 21.0), (20, 1028, 9.5), (64, 516, 4.0), (5, 2052, 40.1), (12, 4100, 50.0)])
+def test_emulated_edge_case_grids_of_the_gpu_suite(emu_bin, tmp_path, n_theta, n_phi, cut_deg):
+    """The very grids, seeds and tables of tests/test_gpu_parity.py::test_small_grids_against_level0 (single ring,
+    theta_cut = pi, R = 0, odd n_theta, n_phi not a multiple of the tiles), so that the cases the GPU suite will
+    run have run in the emulation first."""
+    rng = np.random.default_rng(n_theta * 7919 + n_phi)
+    cut = math.radians(cut_deg)
+    table = rng.standard_normal(37)
+    x32 = rng.standard_normal((n_theta, n_phi)).astype(np.float32)
+    got, log = emulate(emu_bin, tmp_path, x32, table, cut)
+    assert not np.isnan(got).any(), log
+    expect = oracle.convolve(x32, table, cut, level=0 if n_theta * n_phi <= 4096 else 1)
+    rms = math.sqrt((expect ** 2).mean())
+    assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
