@@ -173,3 +173,23 @@ def test_emulated_edge_case_grids_of_the_gpu_suite(emu_bin, tmp_path, n_theta, n
     expect = oracle.convolve(x32, table, cut, level=0 if n_theta * n_phi <= 4096 else 1)
     rms = math.sqrt((expect ** 2).mean())
     assert math.sqrt(((got - expect) ** 2).mean()) / rms <= 1e-6 and float(np.abs(got - expect).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("cfg,k,stride", [(1, 0, 16), (2, 0, 97), (3, 0, 59), (3, 1, 61), (3, 2, 61), (3, 3, 67), (4, 0, 89), (4, 1, 97),
+                                          (4, 2, 101), (4, 3, 211)])
+def test_emulated_subsets_of_the_full_size_schedules(emu_bin, tmp_path, cfg, k, stride):
+    """The REAL schedules of BASELINE configs[1..4] (full-size grids, the workloads' own maps and tables): every
+    `stride`-th work item of the launch bench.py times runs in the emulation - the heaviest polar WIDE item, WIDE and
+    NARROW items of every band, single- and double-buffered weight tables - and its outputs are compared with the oracle."""
+    from paper_1211_3556_b200 import workloads as wl
+    w = wl.config(cfg)[k]
+    x32, table = w.map_f32(), w.table()
+    got, log = emulate(emu_bin, tmp_path, x32, table, w.theta_cut, env={"EMU_ITEM_STRIDE": str(stride)})
+    written = ~np.isnan(got)
+    assert written.any(), log
+    pix = np.flatnonzero(written.reshape(-1))
+    pix = pix[:: max(1, len(pix) // 30000)]
+    expect = oracle.convolve(x32, table, w.theta_cut, level=1, pixels=pix)
+    rms = math.sqrt((got[written] ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
