@@ -40,6 +40,11 @@ constexpr int kNarrowP = 16;
 constexpr int kNarrowSpan = 32 * kNarrowP;           // 512 contiguous phi outputs per warp = per NARROW item
 constexpr int kNarrowTileBytes = 80;
 constexpr int kNarrowSlotBytes = (32 + 2 * (kHaloNarrow / kNarrowP) + 1) * kNarrowTileBytes;
+// A ring's weight block of wcopy floats takes wcopy + kNarrowWPad floats of the shared weight area: the chain
+// prefetches the 8 bytes after a run's last weight, and that read must not land in the neighbouring block, which in
+// the double-buffered case is being filled for the next pass (harmless - the value is never used - but a
+// shared-memory hazard for a race checker all the same).
+constexpr int kNarrowWPad = 4;
 
 // ---- WIDE items (windows of 64 .. n_phi taps): warp-autonomous path ------------------------------
 // A warp owns kWarpSpan contiguous outputs of ONE ring and streams its share of the ring's taps through

@@ -147,18 +147,18 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { emu::cp_async_wait(N); }
 __device__ __forceinline__ void cp_async_wait_all() { emu::cp_async_wait(0); }
 __device__ __forceinline__ void lds128(float& a, float& b, float& c, float& d, const uint32_t addr) {
-    const float* q = reinterpret_cast<const float*>(emu::smem_at(addr, 16));
+    const float* q = reinterpret_cast<const float*>(emu::smem_read(addr, 16));
     a = q[0]; b = q[1]; c = q[2]; d = q[3];
 }
 template <int OFF>
 __device__ __forceinline__ void lds128i(float& a, float& b, float& c, float& d, const uint32_t addr) { lds128(a, b, c, d, addr + (uint32_t)OFF); }
 template <int OFF>
 __device__ __forceinline__ void lds64i(float& a, float& b, const uint32_t addr) {
-    const float* q = reinterpret_cast<const float*>(emu::smem_at(addr + (uint32_t)OFF, 8));
+    const float* q = reinterpret_cast<const float*>(emu::smem_read(addr + (uint32_t)OFF, 8));
     a = q[0]; b = q[1];
 }
 __device__ __forceinline__ void lds128u(int& a, int& b, int& c, int& d, const uint32_t addr) {
-    const int* q = reinterpret_cast<const int*>(emu::smem_at(addr, 16));
+    const int* q = reinterpret_cast<const int*>(emu::smem_read(addr, 16));
     a = q[0]; b = q[1]; c = q[2]; d = q[3];
 }
 #endif
@@ -436,12 +436,13 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
     const int NS = 2 * p.R + 2 * S;                           // row slots
     constexpr int slot_bytes = kNarrowSlotBytes;
     const uint32_t rows = (uint32_t)__cvta_generic_to_shared(smem);
-    // shared memory: row slots | run descriptors [2][S][W] | weight area: [2][S][wcopy] if that fits (the tables of
-    // the next pass are then copied during the current one), else [S][wcopy] (every warp reloads its own ring's
+    // shared memory: row slots | run descriptors [2][S][W] | weight area: [2][S][wstride] if that fits (the tables of
+    // the next pass are then copied during the current one), else [S][wstride] (every warp reloads its own ring's
     // block at the start of a pass; only the polar-most bands of the class, whose blocks are the largest)
     const uint32_t pdbuf_addr = rows + (uint32_t)(NS * slot_bytes);
     const uint32_t wbuf_addr = pdbuf_addr + (uint32_t)(2 * S * W * sizeof(NarrowRun));
-    const bool dbl = 2 * S * it.wcopy <= p.wcap;
+    const int wstride = it.wcopy + kNarrowWPad;
+    const bool dbl = 2 * S * wstride <= p.wcap;
     const int lam0 = it.i0, lam_end = it.i0 + nr;
     const int npass = (nr + S - 1) / S;
 
@@ -473,7 +474,7 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
         const uint32_t pdst = pdbuf_addr + (uint32_t)((tb * W) * sizeof(NarrowRun));
         for (int q = lane; q < W; q += 32) cp_async16(pdst + 16 * q, psrc + q);
         const float* src = p.weights + p.narrow_w_base + (size_t)(lam - p.first_narrow) * p.wslot;
-        const uint32_t dst = wbuf_addr + (uint32_t)((tb * it.wcopy) * 4);
+        const uint32_t dst = wbuf_addr + (uint32_t)((tb * wstride) * 4);
         for (int q = lane; q < n4; q += 32) cp_async16(dst + 16 * q, src + 4 * q);
     };
     for (int q = s; q < 2 * p.R + S; q += S) stage_row(lam0 - p.R + q);
@@ -499,7 +500,7 @@ __device__ void conv_narrow(const ConvParams& p, const Item& it, char* smem, con
 #pragma unroll
             for (int m = 0; m < kNarrowP; m++) { a0[m] = 0.f; a1[m] = 0.f; }
             const int tb = dbl ? (pass & 1) * S + s : s;
-            const uint32_t wring = wbuf_addr + (uint32_t)(tb * it.wcopy * 4);
+            const uint32_t wring = wbuf_addr + (uint32_t)(tb * wstride * 4);
             const uint32_t spd = pdbuf_addr + (uint32_t)(tb * W * sizeof(NarrowRun));
             int slot = (lam - p.R) % NS; if (slot < 0) slot += NS;
             uint32_t zt = rows + (uint32_t)(slot * slot_bytes) + lane_tile;

@@ -144,7 +144,7 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         auto wcap_of = [&](long long budget) { return budget > fixed ? (budget - fixed) / 4 / 4 * 4 : 0ll; };
         auto first_fit = [&](long long wcap, int mult) {           // first ring of the class whose block fits `mult` x kWarps times
             int fn = s.first_narrow;
-            while (fn < s.n_north && (long long)mult * kWarps * (long long)slots[fn] > wcap) fn++;
+            while (fn < s.n_north && (long long)mult * kWarps * (long long)(slots[fn] + kNarrowWPad) > wcap) fn++;
             return fn;
         };
         const long long wcap2 = wcap_of(kSmemTwoPerSm), wcap1 = wcap_of(kSmemBudget);
@@ -161,7 +161,7 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
             for (int i = s.first_narrow; i < s.n_north; i++) wslot = std::max(wslot, slots[i]);
             s.narrow_wslot = (int)wslot;
             // no more shared memory than the largest item needs (double-buffered if it can be)
-            const long long need = std::min<long long>(wcap, 2ll * kWarps * (long long)wslot);
+            const long long need = std::min<long long>(wcap, 2ll * kWarps * (long long)(wslot + kNarrowWPad));
             s.narrow_wcap = (int)need;
             s.smem_narrow = (size_t)(fixed + 4 * need);
         }
@@ -254,7 +254,7 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
     // Two CTAs share an SM, so a band is cut at half the WIDE items' cost cap.
     if (s.first_narrow < s.n_north) {
         constexpr int S = kWarps, L = kNarrowSpan;
-        auto doubles = [&](int i) { return 2ll * S * (long long)s.ring_slots[i] <= (long long)s.narrow_wcap; };
+        auto doubles = [&](int i) { return 2ll * S * (long long)(s.ring_slots[i] + kNarrowWPad) <= (long long)s.narrow_wcap; };
         const int b_min = ((2 * (2 * s.R + S)) + S - 1) / S * S;       // keep the band prologue below ~50 % extra staging
         int i = s.first_narrow;
         while (i < s.n_north) {
@@ -392,7 +392,7 @@ int validate_schedule(const Schedule& s, std::string* why) {
             if (nr < 1 || it.i0 < s.first_narrow || it.i0 + nr > s.n_north) return fail(65, "narrow item band", it.i0, nr);
             if (it.wcopy < 4 || it.wcopy % 4 || it.wcopy > s.narrow_wslot) return fail(66, "narrow item wcopy", it.wcopy, s.narrow_wslot);
             // conv_narrow keeps kWarps (single-buffered) or 2 kWarps (double-buffered) blocks of wcopy floats in the weight area
-            if ((long long)kWarps * it.wcopy > (long long)s.narrow_wcap) return fail(66, "narrow item weight blocks beyond the shared weight area", it.wcopy, s.narrow_wcap);
+            if ((long long)kWarps * (it.wcopy + kNarrowWPad) > (long long)s.narrow_wcap) return fail(66, "narrow item weight blocks beyond the shared weight area", it.wcopy, s.narrow_wcap);
             // stage_ring_tables reads wcopy floats of each ring's block
             if ((long long)s.narrow_w_base + (long long)(it.i0 + nr - 1 - s.first_narrow) * s.narrow_wslot + it.wcopy > wtot) return fail(67, "narrow weight block beyond the buffer", it.i0, nr);
             for (int q = 0; q < nr; q++) {
@@ -455,9 +455,8 @@ size_t wide_smem_bytes(int R) {
 // buffers of S x (2R+1) run descriptors, and a weight area of `wcap` floats
 size_t narrow_smem_bytes(int R, int wcap) {
     constexpr int S = kWarps;
-    // + 16 bytes: the weight prefetch of a chain step reads the 8 bytes after a run's last weights, which for the
-    // last block of a completely filled weight area would otherwise lie beyond the CTA's shared memory
-    return (size_t)(2 * R + 2 * S) * (size_t)kNarrowSlotBytes + 2ull * S * (2 * R + 1) * sizeof(NarrowRun) + 4ull * (size_t)wcap + 16;
+    // (every weight block carries kNarrowWPad floats of its own for the chain's weight prefetch: conv_narrow)
+    return (size_t)(2 * R + 2 * S) * (size_t)kNarrowSlotBytes + 2ull * S * (2 * R + 1) * sizeof(NarrowRun) + 4ull * (size_t)wcap;
 }
 
 }  // namespace arkcos

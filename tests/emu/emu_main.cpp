@@ -39,14 +39,56 @@ static std::vector<Range> g_global;
     std::fprintf(stderr, "EMU FAILURE: %s (%ld, %ld) block %u thread %u\n", what, a, b, t_blockIdx.x, t_threadIdx.x);
     std::_Exit(3);
 }
-void sync_threads() { g_cta_barrier->arrive_and_wait(); }
-void sync_warp() { g_warp_barriers[t_threadIdx.x >> 5]->arrive_and_wait(); }
+static thread_local uint32_t t_cta_epoch = 0, t_warp_epoch = 0;   // barriers this thread has passed (hazard checker below)
+void sync_threads() { g_cta_barrier->arrive_and_wait(); ++t_cta_epoch; }
+void sync_warp() { g_warp_barriers[t_threadIdx.x >> 5]->arrive_and_wait(); ++t_warp_epoch; }
 void check_global(const void* p, size_t bytes) {
     const unsigned char* q = (const unsigned char*)p;
     if ((uintptr_t)q % 16) fail("misaligned global access of cp.async", (long)((uintptr_t)q % 16), (long)bytes);
     for (const Range& r : g_global)
         if (q >= r.lo && q + bytes <= r.hi) return;
     fail("cp.async source outside every global buffer", 0, (long)bytes);
+}
+
+// ---- shared-memory hazard checker -------------------------------------------------------------------
+// What `compute-sanitizer --tool racecheck` reports on the device, for the accesses the emulation sees (the
+// ld.shared wrappers and the cp.async copies): two accesses of one shared-memory word by different threads, at
+// least one a write, with no barrier both threads took part in between them.  Every thread counts the CTA
+// barriers and the warp barriers it has passed; an access by thread b is ordered after an earlier access by
+// thread a iff b has passed a CTA barrier a had not yet passed at its access, or the two are in one warp and b
+// has passed a warp barrier a had not.  A cp.async WRITE may land any time between its issue and its wait: it is
+// checked against earlier readers / writers at issue and becomes the word's writer at the wait.
+struct Stamp { uint16_t tid; uint16_t valid; uint32_t cta_epoch, warp_epoch; };
+static std::vector<Stamp> g_writer, g_reader;                     // per 4-byte word: last writer, most recent reader
+static std::mutex g_shadow_mutex;
+static const bool g_racecheck = std::getenv("EMU_NO_RACECHECK") == nullptr;
+static bool ordered_after(const Stamp& a) {                        // is the calling thread's access ordered after stamp a?
+    if (!a.valid || a.tid == t_threadIdx.x) return true;
+    if (t_cta_epoch > a.cta_epoch) return true;
+    return (a.tid >> 5) == (t_threadIdx.x >> 5) && t_warp_epoch > a.warp_epoch;
+}
+static Stamp now() { return Stamp{(uint16_t)t_threadIdx.x, 1, t_cta_epoch, t_warp_epoch}; }
+void note_read(uint32_t addr, uint32_t bytes) {
+    if (!g_racecheck) return;
+    std::lock_guard<std::mutex> lock(g_shadow_mutex);
+    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
+        if (!ordered_after(g_writer[w])) fail("shared-memory hazard: read of a word another thread wrote without a barrier in between (word, writer)", w, g_writer[w].tid);
+        const Stamp& r = g_reader[w];
+        if (!r.valid || t_cta_epoch >= r.cta_epoch) g_reader[w] = now();
+    }
+}
+static void note_write_issue(uint32_t addr, uint32_t bytes) {
+    if (!g_racecheck) return;
+    std::lock_guard<std::mutex> lock(g_shadow_mutex);
+    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
+        if (!ordered_after(g_reader[w])) fail("shared-memory hazard: cp.async issued into a word another thread may still be reading (word, reader)", w, g_reader[w].tid);
+        if (!ordered_after(g_writer[w])) fail("shared-memory hazard: two unordered writes of one word (word, writer)", w, g_writer[w].tid);
+    }
+}
+static void note_write_done(uint32_t addr, uint32_t bytes) {
+    if (!g_racecheck) return;
+    std::lock_guard<std::mutex> lock(g_shadow_mutex);
+    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) g_writer[w] = now();
 }
 
 struct Pending { uint32_t dst; const void* src; };
@@ -59,12 +101,13 @@ static const bool g_eager = std::getenv("EMU_EAGER") != nullptr;
 void cp_async_enqueue(uint32_t dst, const void* src) {
     (void)smem_at(dst, 16);
     check_global(src, 16);
-    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); return; }
+    note_write_issue(dst, 16);
+    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); note_write_done(dst, 16); return; }
     t_open.push_back(Pending{dst, src});
 }
 void cp_async_commit_group() { t_groups.push_back(std::move(t_open)); t_open.clear(); }
 static void perform(const std::vector<Pending>& g) {
-    for (const Pending& c : g) std::memcpy(smem_at(c.dst, 16), c.src, 16);
+    for (const Pending& c : g) { std::memcpy(smem_at(c.dst, 16), c.src, 16); note_write_done(c.dst, 16); }
 }
 void cp_async_wait(int keep_groups) {
     if (keep_groups == 0) {            // wait_all / wait_group 0: everything, committed or not
@@ -85,6 +128,7 @@ static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_byte
     g_smem_bytes = smem_bytes;
     g_smem = (unsigned char*)std::malloc(smem_bytes ? smem_bytes : 16);
     std::memset(g_smem, 0xFF, smem_bytes);                        // NaN pattern
+    g_writer.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0}); g_reader.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0});
     g_blockDim = dim3(threads);
     g_cta_barrier = std::make_unique<std::barrier<>>((std::ptrdiff_t)threads);
     g_warp_barriers.clear();
@@ -93,6 +137,7 @@ static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_byte
     for (unsigned t = 0; t < threads; t++)
         pool.emplace_back([&, t] {
             t_threadIdx = uint3{t, 0, 0}; t_blockIdx = uint3{bx, by, 0};
+            t_cta_epoch = 0; t_warp_epoch = 0;
             body();
             thread_exit_check();
         });
@@ -111,8 +156,33 @@ static std::vector<T> read_file(const char* path, size_t n) {
     return v;
 }
 
+// Self-test of the hazard checker: tiny two-warp "kernels" with and without the barrier that orders a cp.async
+// write and an ld.shared read.  Modes 1 and 3 must die with EMU FAILURE (exit 3), modes 2 and 4 must pass.
+static int hazard_selftest(int mode) {
+    static float src[8] = {1, 2, 3, 4, 5, 6, 7, 8};
+    emu::g_global = {{(const unsigned char*)src, (const unsigned char*)(src + 8)}};
+    emu::run_cta(0, 0, 64, 64, [&] {
+        const unsigned t = threadIdx.x;
+        float a, b, c, d;
+        if (mode == 1 || mode == 2) {                      // write by thread 0, read by thread 40 (another warp)
+            if (t == 0) { arkcos::cp_async16(0, src); arkcos::cp_async_wait_all(); }
+            if (mode == 2) __syncthreads();
+            if (t == 40) arkcos::lds128(a, b, c, d, 0);
+            if (mode == 1) __syncthreads();                // a barrier AFTER the read does not order it
+        } else {                                           // read by thread 1, then cp.async by thread 2 (same warp)
+            if (t == 1) arkcos::lds128(a, b, c, d, 16);
+            if (mode == 4) __syncwarp();
+            if (t == 2) { arkcos::cp_async16(16, src + 4); arkcos::cp_async_wait_all(); }
+            if (mode == 3) __syncwarp();
+        }
+    });
+    std::printf("selftest %d passed the checker\n", mode);
+    return 0;
+}
+
 int main(int argc, char** argv) {
     using namespace arkcos;
+    if (argc == 3 && std::string(argv[1]) == "selftest") return hazard_selftest(std::atoi(argv[2]));
     if (argc < 8) { std::fprintf(stderr, "usage: emu_arkcos n_theta n_phi theta_cut n_table table.f64 in.f32 out.f32 [only_wide|only_narrow]\n"); return 2; }
     const int n_theta = std::atoi(argv[1]), n_phi = std::atoi(argv[2]);
     const double theta_cut = std::atof(argv[3]);
@@ -174,7 +244,7 @@ int main(int argc, char** argv) {
     if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
     std::fclose(f);
     int n_single = 0;
-    for (size_t b = (size_t)s.n_wide_items; b < s.items.size(); b++) n_single += 2 * kWarps * s.items[b].wcopy > s.narrow_wcap;
+    for (size_t b = (size_t)s.n_wide_items; b < s.items.size(); b++) n_single += 2 * kWarps * (s.items[b].wcopy + kNarrowWPad) > s.narrow_wcap;
     std::printf("single-buffered narrow items %d; ", n_single);
     std::printf("emu ok: R %d first_narrow %d n_north %d items wide %d narrow %d smem wide %zu narrow %zu weight_slots %llu\n", s.R,
                 s.first_narrow, s.n_north, n_wide, n_narrow, s.smem_wide, s.smem_narrow, (unsigned long long)s.weight_slots);

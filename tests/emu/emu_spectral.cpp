@@ -25,6 +25,7 @@ static std::unique_ptr<std::barrier<>> g_cta_barrier;
 void sync_threads() { g_cta_barrier->arrive_and_wait(); }
 void sync_warp() {}
 void check_global(const void*, size_t) {}
+void note_read(uint32_t, uint32_t) {}
 void cp_async_enqueue(uint32_t, const void*) { fail("cp.async is not used by the spectral kernels", 0, 0); }
 void cp_async_commit_group() {}
 void cp_async_wait(int) {}

@@ -45,6 +45,10 @@ static inline unsigned char* smem_at(uint32_t addr, uint32_t bytes) {
     if (addr % bytes) fail("misaligned shared-memory access", addr, bytes);
     return g_smem + addr;
 }
+// shared-memory hazard checker (emu_main.cpp): the CPU counterpart of `compute-sanitizer --tool racecheck` for the
+// accesses that go through the kernels' PTX wrappers (ld.shared reads, cp.async writes)
+void note_read(uint32_t addr, uint32_t bytes);
+static inline unsigned char* smem_read(uint32_t addr, uint32_t bytes) { unsigned char* p = smem_at(addr, bytes); note_read(addr, bytes); return p; }
 void check_global(const void* p, size_t bytes);   // must lie inside a registered global buffer, 16-byte aligned
 // cp.async emulation: copies are queued per thread and only performed by the wait calls
 void cp_async_enqueue(uint32_t dst, const void* src);

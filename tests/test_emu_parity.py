@@ -193,3 +193,16 @@ def test_emulated_subsets_of_the_full_size_schedules(emu_bin, tmp_path, cfg, k, 
     rms = math.sqrt((got[written] ** 2).mean())
     err = got.reshape(-1)[pix] - expect
     assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
+
+
+@pytest.mark.parametrize("mode,must_fail", [(1, True), (2, False), (3, True), (4, False)])
+def test_emulation_hazard_checker_catches_missing_barriers(emu_bin, mode, must_fail):
+    """The emulation's shared-memory hazard checker (the CPU counterpart of compute-sanitizer racecheck for cp.async
+    writes and ld.shared reads): a read of another warp's cp.async data without a CTA barrier, and a cp.async into a
+    word a lane of the same warp has read without a warp barrier, must be reported; with the barrier they must pass.
+    Every other emulation test in this file runs with the checker on."""
+    res = subprocess.run([emu_bin, "selftest", str(mode)], capture_output=True, text=True, timeout=60)
+    if must_fail:
+        assert res.returncode == 3 and "shared-memory hazard" in res.stderr, (res.returncode, res.stdout, res.stderr)
+    else:
+        assert res.returncode == 0, res.stderr
