@@ -28,6 +28,13 @@ arkcos_status arkcos_measure_convolve(const arkcos_plan *plan, const float *d_in
                                       void *stream, float *ms_generate, float *ms_convolve);
 
 /*
+ * arkcos_plan_reserve_host_io_chunks - as arkcos_plan_reserve_host_io (include/arkcos.h), with the number of ring
+ * bands of the arkcos_convolve_host pipeline given instead of derived from the map size (0 = derive it; clamped to
+ * n_theta).  For tests of the pipeline on small maps and for tuning.  No effect once the staging is reserved.
+ */
+arkcos_status arkcos_plan_reserve_host_io_chunks(arkcos_plan *plan, int n_chunks);
+
+/*
  * arkcos_plan_item - work item `index` (0 .. arkcos_plan_info.n_items - 1) of the convolution launch, in launch
  * order (heaviest first), so that tests can probe the seams of the schedule.  fields[6] receives:
  *   [0] class: 0 = WIDE (one output ring), 1 = NARROW (a band of rings of one hemisphere)

@@ -56,6 +56,7 @@ SYMBOLS = [
     ("arkcos_convolve_batch", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]),
     ("arkcos_convolve_host", ctypes.c_int, [_c_plan_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     ("arkcos_plan_reserve_host_io", ctypes.c_int, [_c_plan_p]),
+    ("arkcos_plan_reserve_host_io_chunks", ctypes.c_int, [_c_plan_p, ctypes.c_int]),
     ("arkcos_plan_destroy", ctypes.c_int, [_c_plan_p]),
     ("arkcos_status_string", ctypes.c_char_p, [ctypes.c_int]),
     ("arkcos_last_cuda_error", ctypes.c_char_p, []),
@@ -147,8 +148,8 @@ class Plan:
         _check(lib().arkcos_convolve_spectral(self._h, _ptr(d_in), _ptr(d_out), int(n_maps), d_work.data_ptr(),
                                               int(d_work.numel() * d_work.element_size()), stream), "arkcos_convolve_spectral")
 
-    def reserve_host_io(self):
-        _check(lib().arkcos_plan_reserve_host_io(self._h), "arkcos_plan_reserve_host_io")
+    def reserve_host_io(self, n_chunks: int = 0):
+        _check(lib().arkcos_plan_reserve_host_io_chunks(self._h, int(n_chunks)), "arkcos_plan_reserve_host_io")
 
     def measure_convolve(self, d_in, d_out, stream: int = 0, n_maps: int = 1) -> Tuple[float, float]:
         a, b = ctypes.c_float(0), ctypes.c_float(0)

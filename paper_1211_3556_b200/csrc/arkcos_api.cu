@@ -1,7 +1,13 @@
 // arkcos_api.cu - the C ABI of include/arkcos.h: plan creation (S1 + uploads), the hot-path launches
 // (S2 weight generator, S3 convolution) and the introspection / measurement hooks.
 // Product code; shares nothing with oracle/.  No CPU fallback: compute entry points need a CUDA device.
+#ifdef ARKCOS_HOST_EMU
+#include "emu_runtime.h"   // tests/emu: the CUDA runtime emulated on the host (test builds only, never the product)
+#define ARKCOS_LAUNCH(kernel, grid, block, smem, stream, params) emu::launch(kernel, dim3(grid), dim3(block), (size_t)(smem), params)
+#else
 #include <cuda_runtime.h>
+#define ARKCOS_LAUNCH(kernel, grid, block, smem, stream, params) kernel<<<grid, block, smem, stream>>>(params)
+#endif
 
 #include <algorithm>
 #include <cmath>
@@ -90,7 +96,7 @@ arkcos_status launch_generate(const arkcos_plan* pl, cudaStream_t st) {
         g.t_scale2 = (double)(pl->n_table - 1 - pl->m_split) / (pl->sched.theta_cut - pl->theta_split);
     }
     g.table_in_smem = pl->table_in_smem;
-    k_generate_weights<<<pl->gen_grid, kGenThreads, pl->gen_smem, st>>>(g);
+    ARKCOS_LAUNCH(k_generate_weights, pl->gen_grid, kGenThreads, pl->gen_smem, st, g);
     CU(cudaGetLastError());
     return ARKCOS_OK;
 }
@@ -112,12 +118,12 @@ arkcos_status launch_items(const arkcos_plan* pl, ConvParams c, const Item* wide
     if (pl->flags & ARKCOS_PLAN_ONLY_WIDE) n_narrow = 0;
     if (n_wide > 0) {
         c.items = wide;
-        k_convolve_wide<<<dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st>>>(c);
+        ARKCOS_LAUNCH(k_convolve_wide, dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st, c);
         CU(cudaGetLastError());
     }
     if (n_narrow > 0) {
         c.items = narrow;
-        k_convolve_narrow<<<dim3((unsigned)n_narrow, (unsigned)n_maps, 1), kThreads, pl->sched.smem_narrow, st>>>(c);
+        ARKCOS_LAUNCH(k_convolve_narrow, dim3((unsigned)n_narrow, (unsigned)n_maps, 1), kThreads, pl->sched.smem_narrow, st, c);
         CU(cudaGetLastError());
     }
     return ARKCOS_OK;
@@ -180,7 +186,7 @@ arkcos_status build_spectral(arkcos_plan* pl) {
             !cuda_ok(cudaFuncSetAttribute(k_spectral_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, kSpecMaxPhi * 10 + 16),
                      "cudaFuncSetAttribute(k_spectral_apply)")) { st = ARKCOS_ECUDA; break; }
         const int grid = std::min<int>((int)sp.size(), 8 * std::max(1, pl->sm_count));
-        k_spectral_weights<<<grid, kSpecThreads, smem, 0>>>(w);
+        ARKCOS_LAUNCH(k_spectral_weights, grid, kSpecThreads, smem, 0, w);
         if (!cuda_ok(cudaGetLastError(), "k_spectral_weights") || !cuda_ok(cudaDeviceSynchronize(), "k_spectral_weights sync")) { st = ARKCOS_ECUDA; break; }
     } while (0);
     cudaFree(d_sp); cudaFree(d_cos);
@@ -376,13 +382,15 @@ arkcos_status arkcos_measure_convolve(const arkcos_plan* pl, const float* d_in, 
     return ARKCOS_OK;
 }
 
-arkcos_status arkcos_plan_reserve_host_io(arkcos_plan* pl) {
-    if (!pl) return ARKCOS_EINVAL;
+arkcos_status arkcos_plan_reserve_host_io(arkcos_plan* pl) { return arkcos_plan_reserve_host_io_chunks(pl, 0); }
+
+arkcos_status arkcos_plan_reserve_host_io_chunks(arkcos_plan* pl, int n_chunks) {
+    if (!pl || n_chunks < 0) return ARKCOS_EINVAL;
     if (pl->flags & ARKCOS_PLAN_HOST_ONLY) return ARKCOS_EUNSUPPORTED;
     if (pl->d_io_in) return ARKCOS_OK;
     const size_t bytes = (size_t)pl->sched.n_theta * pl->sched.n_phi * sizeof(float);
     // chunks of about 8 MB: long enough for the copy engines, short enough that compute and the copy back start early
-    const int n_chunks = (int)std::max<size_t>(1, std::min<size_t>(16, bytes / (8u << 20)));
+    if (n_chunks == 0) n_chunks = (int)std::max<size_t>(1, std::min<size_t>(16, bytes / (8u << 20)));
     arkcos_status st = ARKCOS_OK;
     try { build_pipeline(pl->sched, n_chunks, pl->pipe); } catch (const std::bad_alloc&) { return ARKCOS_ENOMEM; }
     cudaError_t e = cudaMalloc((void**)&pl->d_io_in, bytes);
@@ -467,9 +475,9 @@ arkcos_status arkcos_convolve_spectral(const arkcos_plan* pl, const float* d_in,
     p.tw_h = pl->d_tw_h; p.tw_n = pl->d_tw_n; p.n_theta = s.n_theta; p.n_phi = s.n_phi; p.R = s.R;
     const dim3 grid((unsigned)s.n_theta, (unsigned)n_maps, 1);
     cudaStream_t cs = (cudaStream_t)stream;
-    k_rfft_rings<<<grid, kSpecThreads, (size_t)(2 * h + h / 2) * sizeof(float2), cs>>>(p);
+    ARKCOS_LAUNCH(k_rfft_rings, grid, kSpecThreads, (size_t)(2 * h + h / 2) * sizeof(float2), cs, p);
     CU(cudaGetLastError());
-    k_spectral_apply<<<grid, kSpecThreads, (size_t)(2 * h + 1 + h / 2) * sizeof(float2), cs>>>(p);
+    ARKCOS_LAUNCH(k_spectral_apply, grid, kSpecThreads, (size_t)(2 * h + 1 + h / 2) * sizeof(float2), cs, p);
     CU(cudaGetLastError());
     return ARKCOS_OK;
 }

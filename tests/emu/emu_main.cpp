@@ -14,138 +14,11 @@
 //
 // It does not replace the GPU parity tests: it checks the index logic (windows, staging, wrap-around,
 // pass structure, weight layout), not the compiled SASS.
-#include <barrier>
-#include <memory>
-#include <mutex>
-#include <thread>
-
-#include "cuda_runtime.h"
+#include "emu_runtime.h"
 
 #include "arkcos_internal.h"
 #include "arkcos_kernels.cuh"
 
-namespace emu {
-thread_local uint3 t_threadIdx, t_blockIdx;
-dim3 g_blockDim, g_gridDim;
-unsigned char* g_smem = nullptr;
-size_t g_smem_bytes = 0;
-
-static std::unique_ptr<std::barrier<>> g_cta_barrier;
-static std::vector<std::unique_ptr<std::barrier<>>> g_warp_barriers;
-struct Range { const unsigned char* lo; const unsigned char* hi; };
-static std::vector<Range> g_global;
-
-[[noreturn]] void fail(const char* what, long a, long b) {
-    std::fprintf(stderr, "EMU FAILURE: %s (%ld, %ld) block %u thread %u\n", what, a, b, t_blockIdx.x, t_threadIdx.x);
-    std::_Exit(3);
-}
-static thread_local uint32_t t_cta_epoch = 0, t_warp_epoch = 0;   // barriers this thread has passed (hazard checker below)
-void sync_threads() { g_cta_barrier->arrive_and_wait(); ++t_cta_epoch; }
-void sync_warp() { g_warp_barriers[t_threadIdx.x >> 5]->arrive_and_wait(); ++t_warp_epoch; }
-void check_global(const void* p, size_t bytes) {
-    const unsigned char* q = (const unsigned char*)p;
-    if ((uintptr_t)q % 16) fail("misaligned global access of cp.async", (long)((uintptr_t)q % 16), (long)bytes);
-    for (const Range& r : g_global)
-        if (q >= r.lo && q + bytes <= r.hi) return;
-    fail("cp.async source outside every global buffer", 0, (long)bytes);
-}
-
-// ---- shared-memory hazard checker -------------------------------------------------------------------
-// What `compute-sanitizer --tool racecheck` reports on the device, for the accesses the emulation sees (the
-// ld.shared wrappers and the cp.async copies): two accesses of one shared-memory word by different threads, at
-// least one a write, with no barrier both threads took part in between them.  Every thread counts the CTA
-// barriers and the warp barriers it has passed; an access by thread b is ordered after an earlier access by
-// thread a iff b has passed a CTA barrier a had not yet passed at its access, or the two are in one warp and b
-// has passed a warp barrier a had not.  A cp.async WRITE may land any time between its issue and its wait: it is
-// checked against earlier readers / writers at issue and becomes the word's writer at the wait.
-struct Stamp { uint16_t tid; uint16_t valid; uint32_t cta_epoch, warp_epoch; };
-static std::vector<Stamp> g_writer, g_reader;                     // per 4-byte word: last writer, most recent reader
-static std::mutex g_shadow_mutex;
-static const bool g_racecheck = std::getenv("EMU_NO_RACECHECK") == nullptr;
-static bool ordered_after(const Stamp& a) {                        // is the calling thread's access ordered after stamp a?
-    if (!a.valid || a.tid == t_threadIdx.x) return true;
-    if (t_cta_epoch > a.cta_epoch) return true;
-    return (a.tid >> 5) == (t_threadIdx.x >> 5) && t_warp_epoch > a.warp_epoch;
-}
-static Stamp now() { return Stamp{(uint16_t)t_threadIdx.x, 1, t_cta_epoch, t_warp_epoch}; }
-void note_read(uint32_t addr, uint32_t bytes) {
-    if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
-    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
-        if (!ordered_after(g_writer[w])) fail("shared-memory hazard: read of a word another thread wrote without a barrier in between (word, writer)", w, g_writer[w].tid);
-        const Stamp& r = g_reader[w];
-        if (!r.valid || t_cta_epoch >= r.cta_epoch) g_reader[w] = now();
-    }
-}
-static void note_write_issue(uint32_t addr, uint32_t bytes) {
-    if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
-    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
-        if (!ordered_after(g_reader[w])) fail("shared-memory hazard: cp.async issued into a word another thread may still be reading (word, reader)", w, g_reader[w].tid);
-        if (!ordered_after(g_writer[w])) fail("shared-memory hazard: two unordered writes of one word (word, writer)", w, g_writer[w].tid);
-    }
-}
-static void note_write_done(uint32_t addr, uint32_t bytes) {
-    if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
-    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) g_writer[w] = now();
-}
-
-struct Pending { uint32_t dst; const void* src; };
-static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
-static thread_local std::vector<Pending> t_open;                  // not yet committed
-// Two modes bracket what the hardware may do with a cp.async: DEFERRED (default) performs the copy only at
-// the wait - a read before the wait sees stale data (RAW hazard); EAGER (EMU_EAGER=1) performs it at once - a
-// copy into a buffer that other threads still read clobbers it (WAR hazard).
-static const bool g_eager = std::getenv("EMU_EAGER") != nullptr;
-void cp_async_enqueue(uint32_t dst, const void* src) {
-    (void)smem_at(dst, 16);
-    check_global(src, 16);
-    note_write_issue(dst, 16);
-    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); note_write_done(dst, 16); return; }
-    t_open.push_back(Pending{dst, src});
-}
-void cp_async_commit_group() { t_groups.push_back(std::move(t_open)); t_open.clear(); }
-static void perform(const std::vector<Pending>& g) {
-    for (const Pending& c : g) { std::memcpy(smem_at(c.dst, 16), c.src, 16); note_write_done(c.dst, 16); }
-}
-void cp_async_wait(int keep_groups) {
-    if (keep_groups == 0) {            // wait_all / wait_group 0: everything, committed or not
-        for (auto& g : t_groups) perform(g);
-        t_groups.clear();
-        perform(t_open); t_open.clear();
-        return;
-    }
-    while ((int)t_groups.size() > keep_groups) { perform(t_groups.front()); t_groups.erase(t_groups.begin()); }
-}
-static void thread_exit_check() {
-    if (!t_open.empty() || !t_groups.empty()) fail("thread exits with cp.async copies it never waited for", (long)t_groups.size(), 0);
-}
-
-// run one CTA of `threads` threads
-template <typename F>
-static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_bytes, F&& body) {
-    g_smem_bytes = smem_bytes;
-    g_smem = (unsigned char*)std::malloc(smem_bytes ? smem_bytes : 16);
-    std::memset(g_smem, 0xFF, smem_bytes);                        // NaN pattern
-    g_writer.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0}); g_reader.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0});
-    g_blockDim = dim3(threads);
-    g_cta_barrier = std::make_unique<std::barrier<>>((std::ptrdiff_t)threads);
-    g_warp_barriers.clear();
-    for (unsigned w = 0; w < threads / 32; w++) g_warp_barriers.push_back(std::make_unique<std::barrier<>>(32));
-    std::vector<std::thread> pool;
-    for (unsigned t = 0; t < threads; t++)
-        pool.emplace_back([&, t] {
-            t_threadIdx = uint3{t, 0, 0}; t_blockIdx = uint3{bx, by, 0};
-            t_cta_epoch = 0; t_warp_epoch = 0;
-            body();
-            thread_exit_check();
-        });
-    for (auto& th : pool) th.join();
-    std::free(g_smem);
-    g_smem = nullptr;
-}
-}  // namespace emu
 
 template <typename T>
 static std::vector<T> read_file(const char* path, size_t n) {

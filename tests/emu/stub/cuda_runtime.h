@@ -31,6 +31,22 @@ static inline float2 make_float2(float a, float b) { return float2{a, b}; }
 using std::max;
 using std::min;
 
+// ---- the part of the CUDA runtime API the library's API layer uses (implemented in emu_runtime.h) ----
+#include <chrono>
+typedef int cudaError_t;
+enum { cudaSuccess = 0, cudaErrorInvalidValue = 1, cudaErrorMemoryAllocation = 2 };
+enum { cudaMemcpyHostToDevice = 1, cudaMemcpyDeviceToHost = 2 };
+enum { cudaFuncAttributeMaxDynamicSharedMemorySize = 8, cudaFuncAttributePreferredSharedMemoryCarveout = 9, cudaSharedmemCarveoutMaxShared = 100 };
+enum { cudaStreamNonBlocking = 1, cudaEventDisableTiming = 2 };
+namespace emu {
+struct Event { double t; };
+struct Stream {};
+static inline double wall_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
+}
+typedef emu::Event* cudaEvent_t;
+typedef emu::Stream* cudaStream_t;
+struct cudaDeviceProp { int major, minor, multiProcessorCount; };
+
 namespace emu {
 extern thread_local uint3 t_threadIdx, t_blockIdx;
 extern dim3 g_blockDim, g_gridDim;
@@ -62,4 +78,5 @@ void cp_async_wait(int keep_groups);
 #define gridDim (emu::g_gridDim)
 static inline void __syncthreads() { emu::sync_threads(); }
 static inline void __syncwarp() { emu::sync_warp(); }
+static inline double __ldg(const double* p) { return *p; }
 static inline size_t __cvta_generic_to_shared(const void* p) { return (size_t)((const unsigned char*)p - emu::g_smem); }
