@@ -152,6 +152,9 @@ def sc_entry_points_bit_identical():
                 assert (h_out == single[0]).all(), chunks
         gen_ms, conv_ms = plan.measure_convolve(d_in[0], again[0], 0)
         assert gen_ms > 0 and conv_ms > 0 and (again[0] == single[0]).all()
+        batch[...] = np.nan
+        gen_ms, conv_ms = plan.measure_convolve(d_in, batch, 0, 3)           # what bench.py times for configs[4]
+        assert gen_ms > 0 and conv_ms > 0 and (batch == single).all()
         st, why = plan.validate()
         assert st == arkcos.OK, why
         assert len(plan.items()) == plan.info().n_items
