@@ -77,13 +77,22 @@ static void note_write_issue(uint32_t addr, uint32_t bytes) {
         if (!ordered_after(g_writer[w])) fail("shared-memory hazard: two unordered writes of one word (word, writer)", w, g_writer[w].tid);
     }
 }
-static void note_write_done(uint32_t addr, uint32_t bytes) {
+// The copy may have landed at any time since its issue: a reader that is not ordered BEFORE the issue (it read while
+// the copy was in flight, with or without a barrier after the issue) is a hazard too.  `ic`, `iw` = the writer's
+// barrier counts at issue.
+static void note_write_done(uint32_t addr, uint32_t bytes, uint32_t ic, uint32_t iw) {
     if (!g_racecheck) return;
     std::lock_guard<std::mutex> lock(g_shadow_mutex);
-    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) g_writer[w] = now();
+    for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
+        const Stamp& r = g_reader[w];
+        const bool before_issue = !r.valid || r.tid == t_threadIdx.x || ic > r.cta_epoch ||
+                                  ((r.tid >> 5) == (t_threadIdx.x >> 5) && iw > r.warp_epoch);
+        if (!before_issue) fail("shared-memory hazard: a word was read by another thread while a cp.async into it was in flight (word, reader)", w, r.tid);
+        g_writer[w] = now();
+    }
 }
 
-struct Pending { uint32_t dst; const void* src; };
+struct Pending { uint32_t dst; const void* src; uint32_t ic, iw; };
 static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
 static thread_local std::vector<Pending> t_open;                  // not yet committed
 // Two modes bracket what the hardware may do with a cp.async: DEFERRED (default) performs the copy only at
@@ -94,12 +103,12 @@ void cp_async_enqueue(uint32_t dst, const void* src) {
     (void)smem_at(dst, 16);
     check_global(src, 16);
     note_write_issue(dst, 16);
-    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); note_write_done(dst, 16); return; }
-    t_open.push_back(Pending{dst, src});
+    if (g_eager) { std::memcpy(smem_at(dst, 16), src, 16); note_write_done(dst, 16, t_cta_epoch, t_warp_epoch); return; }
+    t_open.push_back(Pending{dst, src, t_cta_epoch, t_warp_epoch});
 }
 void cp_async_commit_group() { t_groups.push_back(std::move(t_open)); t_open.clear(); }
 static void perform(const std::vector<Pending>& g) {
-    for (const Pending& c : g) { std::memcpy(smem_at(c.dst, 16), c.src, 16); note_write_done(c.dst, 16); }
+    for (const Pending& c : g) { std::memcpy(smem_at(c.dst, 16), c.src, 16); note_write_done(c.dst, 16, c.ic, c.iw); }
 }
 void cp_async_wait(int keep_groups) {
     if (keep_groups == 0) {            // wait_all / wait_group 0: everything, committed or not

@@ -26,7 +26,7 @@ EMU_BIN = os.path.join(EMU_DIR, "emu_arkcos")
 def emu_bin():
     srcs = [os.path.join(EMU_DIR, "emu_main.cpp"), os.path.join(CSRC, "arkcos_schedule.cpp")]
     deps = srcs + [os.path.join(CSRC, "arkcos_kernels.cuh"), os.path.join(CSRC, "arkcos_internal.h"),
-                   os.path.join(EMU_DIR, "stub", "cuda_runtime.h")]
+                   os.path.join(EMU_DIR, "stub", "cuda_runtime.h"), os.path.join(EMU_DIR, "emu_runtime.h")]
     if not os.path.exists(EMU_BIN) or any(os.path.getmtime(d) > os.path.getmtime(EMU_BIN) for d in deps):
         cmd = ["g++", "-std=c++20", "-O1", "-g", "-fsanitize=address", "-fno-omit-frame-pointer", "-pthread",
                "-DARKCOS_HOST_EMU", "-Wno-unknown-pragmas", "-I", os.path.join(EMU_DIR, "stub"), "-I", CSRC] + srcs + ["-o", EMU_BIN]
