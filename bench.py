@@ -172,7 +172,7 @@ def workload_config(w: wl.Workload):
 
 
 def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
-            only: str = "all", path: str = "direct"):
+            only: str = "all", path: str = "direct", wide_tensor: bool = False):
     """One step = S2 + S3 over ALL maps of the workload (configs[4]: the batch of 8 through arkcos_convolve_batch).
     path = "spectral": the N2 cross-check path (arkcos_convolve_spectral) instead; its step has no S2 (the weight
     spectra are plan-time) and is timed as a whole."""
@@ -191,6 +191,8 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
     spectral = path == "spectral"
     if spectral:
         flags |= arkcos.PLAN_SPECTRAL
+    if wide_tensor:                                     # N1(a) experiment: WIDE items through k_convolve_wide_tc
+        flags |= arkcos.PLAN_WIDE_TENSOR
     plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
@@ -352,6 +354,9 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="five-config report + cost-vs-theta_cut curve")
     ap.add_argument("--path", default="direct", choices=["direct", "spectral"],
                     help="direct = the product's hot path (S2 + S3); spectral = the N2 cross-check path (arkcos_convolve_spectral)")
+    ap.add_argument("--wide-tensor", action="store_true",
+                    help="N1(a) experiment: the WIDE work items on the tensor cores (mma.m16n8k8 TF32, 3-term split; "
+                         "ARKCOS_PLAN_WIDE_TENSOR) instead of the default FFMA kernel; the line says so in config.wide_path")
     ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
                     help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
                          "prints a per-class line, not the bench line)")
@@ -375,19 +380,21 @@ def main():
 
     if args.only != "all":
         if rank == 0:
-            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only)
+            res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only,
+                          wide_tensor=args.wide_tensor)
             info = res["info"]
             slots = int(info.fma_slots_wide) if args.only == "wide" else int(info.fma_slots) - int(info.fma_slots_wide)
             slots *= res["n_maps"]
             peak = res["sm_count"] * FP32_LANES_PER_SM * res["sm_max_mhz"] * 1e6
             print(json.dumps({"report": "class_only", "only": args.only, "workload": w.name, "items": int(info.n_items),
+                              "wide_path": "tensor (k_convolve_wide_tc)" if args.wide_tensor else "ffma (k_convolve_wide)",
                               "convolve_ms": res["conv_ms"], "fma_slots": slots,
                               "issued_lane_frac": slots / (res["conv_ms"] * 1e-3) / peak, "clocks": res["clocks"]}), flush=True)
         if dist is not None:
             dist.destroy_process_group()
         return 0
 
-    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, path=args.path)
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, path=args.path, wide_tensor=args.wide_tensor)
     units = float(res["info"].pair_evals) * res["n_maps"] * args.steps
     total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
     if rank == 0:
@@ -395,6 +402,10 @@ def main():
         line = build_line(w, args, res, world, total_ms, total_units, cpu)
         if args.path == "spectral":
             spectral_line(line, w, res)
+        if args.wide_tensor:
+            line["config"]["wide_path"] = "tensor cores: k_convolve_wide_tc, mma.m16n8k8 TF32 x 3-term split (N1(a) experiment, not the default)"
+            line["roofline"]["kernel"] = "k_convolve_wide_tc + k_convolve_narrow"
+            line["roofline"]["note"] = "useful FP32-equivalent FMAs against the FP32 FFMA peak; the WIDE items run on the tensor pipe"
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

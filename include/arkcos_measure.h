@@ -18,6 +18,14 @@ extern "C" {
 #define ARKCOS_PLAN_ONLY_WIDE 4u
 #define ARKCOS_PLAN_ONLY_NARROW 8u
 
+/* Flag of arkcos_plan_create_ex, EXPERIMENT N1(a) (north_star: tensor cores only "if a ring-pair
+ * circulant is recast as a genuinely dense contraction and ncu shows that it wins"): the WIDE work items run on the
+ * tensor cores - per stage a banded-Toeplitz GEMM with warp-level mma.m16n8k8 TF32 instructions and a 3-term
+ * hi/lo split of both operands that keeps FP32 accuracy (csrc/arkcos_tensor.cuh) - instead of the FFMA kernel.
+ * Same plan, same work items, same weights; the result differs from the default path by FP32 rounding only and
+ * meets the same tolerance against the oracle.  The NARROW items are not affected. */
+#define ARKCOS_PLAN_WIDE_TENSOR 32u
+
 /*
  * arkcos_measure_convolve - one arkcos_convolve_batch on `stream` with CUDA events (created and destroyed
  * inside the call) around each kernel; synchronises the stream and returns the device time of the weight

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libarkcos.so")
 SOURCES = ["arkcos_api.cu", "arkcos_schedule.cpp", "arkcos_split.cpp"]
-HEADERS = ["arkcos_internal.h", "arkcos_kernels.cuh", "arkcos_spectral.cuh", os.path.join("..", "..", "include", "arkcos.h"),
+HEADERS = ["arkcos_internal.h", "arkcos_kernels.cuh", "arkcos_spectral.cuh", "arkcos_tensor.cuh", os.path.join("..", "..", "include", "arkcos.h"),
            os.path.join("..", "..", "include", "arkcos_split.h"), os.path.join("..", "..", "include", "arkcos_measure.h"),
            os.path.join("..", "..", "include", "arkcos_spectral.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

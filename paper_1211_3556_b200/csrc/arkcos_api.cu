@@ -23,6 +23,7 @@
 #include "arkcos_internal.h"
 #include "arkcos_kernels.cuh"
 #include "arkcos_spectral.cuh"
+#include "arkcos_tensor.cuh"
 
 using namespace arkcos;
 
@@ -118,7 +119,10 @@ arkcos_status launch_items(const arkcos_plan* pl, ConvParams c, const Item* wide
     if (pl->flags & ARKCOS_PLAN_ONLY_WIDE) n_narrow = 0;
     if (n_wide > 0) {
         c.items = wide;
-        ARKCOS_LAUNCH(k_convolve_wide, dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st, c);
+        if (pl->flags & ARKCOS_PLAN_WIDE_TENSOR)                  // N1(a): the same items on the tensor cores
+            ARKCOS_LAUNCH(k_convolve_wide_tc, dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st, c);
+        else
+            ARKCOS_LAUNCH(k_convolve_wide, dim3((unsigned)n_wide, (unsigned)n_maps, 1), kThreads, pl->sched.smem_wide, st, c);
         CU(cudaGetLastError());
     }
     if (n_narrow > 0) {
@@ -260,7 +264,8 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
     if (m_split > 0 && (m_split > n_table - 2 || !(theta_split > 0.0) || !(theta_split < theta_cut))) return ARKCOS_EINVAL;
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
-    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_SPECTRAL)) return ARKCOS_EINVAL;
+    if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_SPECTRAL |
+                  ARKCOS_PLAN_WIDE_TENSOR)) return ARKCOS_EINVAL;
     if ((flags & ARKCOS_PLAN_SPECTRAL) && (n_phi < 16 || n_phi > kSpecMaxPhi || (n_phi & (n_phi - 1)) != 0)) return ARKCOS_EUNSUPPORTED;
     if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
@@ -309,6 +314,8 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
         // smaller plan must not lower it under an earlier plan's launches).
         if (!cuda_ok(cudaFuncSetAttribute(k_convolve_wide, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
                      "cudaFuncSetAttribute(k_convolve_wide)") ||
+            !cuda_ok(cudaFuncSetAttribute(k_convolve_wide_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
+                     "cudaFuncSetAttribute(k_convolve_wide_tc)") ||
             !cuda_ok(cudaFuncSetAttribute(k_convolve_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget),
                      "cudaFuncSetAttribute(k_convolve_narrow)") ||
             // two NARROW CTAs of up to kSmemTwoPerSm share an SM only with the largest shared-memory carve-out

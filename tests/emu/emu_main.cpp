@@ -18,6 +18,7 @@
 
 #include "arkcos_internal.h"
 #include "arkcos_kernels.cuh"
+#include "arkcos_tensor.cuh"
 
 
 template <typename T>
@@ -101,13 +102,15 @@ int main(int argc, char** argv) {
     int n_wide = 0, n_narrow = 0;
     // EMU_ITEM_STRIDE=n: run every n-th work item only (big grids; outputs of the skipped items stay NaN)
     const size_t item_stride = std::getenv("EMU_ITEM_STRIDE") ? (size_t)std::atoi(std::getenv("EMU_ITEM_STRIDE")) : 1;
+    const bool wide_tensor = std::getenv("EMU_WIDE_TENSOR") != nullptr;   // WIDE items through k_convolve_wide_tc
     for (size_t b = 0; b < s.items.size(); b++) {
         const bool wide = s.items[b].kind == kWide;
         if (item_stride > 1 && b % item_stride != 0) continue;
         if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
         (wide ? n_wide : n_narrow)++;
         ConvParams cc = c;                                     // each kernel is launched on its own part of the work list
-        if (wide) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide(cc); });
+        if (wide && wide_tensor) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide_tc(cc); });   // N1(a)
+        else if (wide) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide(cc); });
         else {
             cc.items = c.items + s.n_wide_items;
             emu::run_cta((unsigned)(b - s.n_wide_items), 0, kThreads, s.smem_narrow, [&] { k_convolve_narrow(cc); });

@@ -92,6 +92,38 @@ static void note_write_done(uint32_t addr, uint32_t bytes, uint32_t ic, uint32_t
     }
 }
 
+void note_store(uint32_t addr, uint32_t bytes) {                  // plain st.shared: issue and completion coincide
+    note_write_issue(addr, bytes);
+    note_write_done(addr, bytes, t_cta_epoch, t_warp_epoch);
+}
+
+// ---- mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 -------------------------------------------------
+// The 32 threads of a warp publish their fragment registers, meet, and each computes its four elements of
+// D = A B + C from the fragment layout of the PTX ISA ("Matrix Fragments for mma.m16n8k8", .tf32; g = lane >> 2,
+// t = lane & 3):  A[g + 8 (r & 1)][t + 4 (r >> 1)] = a_r,  B[t + 4 r][g] = b_r,  C[g + 8 (r >> 1)][2 t + (r & 1)] = c_r.
+// The tensor core reads the upper 19 bits of an operand register (the 13 low mantissa bits are ignored), forms
+// the products exactly and adds them to C with TRUNCATION; here: exact sum in FP64, then rounded toward zero to FP32.
+// The meeting uses the warp's barrier WITHOUT counting it for the hazard checker: mma.sync converges the warp but
+// orders no shared-memory access.
+static uint32_t g_mma_a[64][32][4], g_mma_b[64][32][2];
+void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+    const unsigned warp = t_threadIdx.x >> 5, lane = t_threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    uint32_t (&A)[32][4] = g_mma_a[warp]; uint32_t (&B)[32][2] = g_mma_b[warp];
+    A[lane][0] = a0; A[lane][1] = a1; A[lane][2] = a2; A[lane][3] = a3; B[lane][0] = b0; B[lane][1] = b1;
+    g_warp_barriers[warp]->arrive_and_wait();
+    auto tf32 = [](uint32_t u) { u &= 0xFFFFE000u; float f; std::memcpy(&f, &u, 4); return (double)f; };
+    for (int r = 0; r < 4; r++) {
+        const unsigned m = g + 8 * (r >> 1), n = 2 * t + (r & 1);
+        double sum = (double)c[r];
+        for (unsigned k = 0; k < 8; k++)
+            sum += tf32(A[(m & 7) * 4 + (k & 3)][(m >> 3) + 2 * (k >> 2)]) * tf32(B[n * 4 + (k & 3)][k >> 2]);
+        float f = (float)sum;                                     // round to nearest, then step back if that rounded away from zero
+        if (std::fabs((double)f) > std::fabs(sum)) f = std::nextafterf(f, 0.0f);
+        c[r] = f;
+    }
+    g_warp_barriers[warp]->arrive_and_wait();
+}
+
 struct Pending { uint32_t dst; const void* src; uint32_t ic, iw; };
 static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
 static thread_local std::vector<Pending> t_open;                  // not yet committed

@@ -25,7 +25,7 @@ DEG = math.pi / 180.0
 
 def build_emu_library():
     srcs = [os.path.join(HERE, "emu_api.cpp"), os.path.join(CSRC, "arkcos_schedule.cpp"), os.path.join(CSRC, "arkcos_split.cpp")]
-    deps = srcs + [os.path.join(CSRC, f) for f in ("arkcos_api.cu", "arkcos_kernels.cuh", "arkcos_spectral.cuh", "arkcos_internal.h")] + \
+    deps = srcs + [os.path.join(CSRC, f) for f in ("arkcos_api.cu", "arkcos_kernels.cuh", "arkcos_spectral.cuh", "arkcos_tensor.cuh", "arkcos_internal.h")] + \
         [os.path.join(HERE, "emu_runtime.h"), os.path.join(HERE, "stub", "cuda_runtime.h")]
     if os.path.exists(LIB) and all(os.path.getmtime(d) <= os.path.getmtime(LIB) for d in deps):
         return LIB
@@ -251,6 +251,34 @@ def sc_class_only_flags():
     ww, nw = ~np.isnan(wide), ~np.isnan(narrow)
     assert (ww ^ nw).all() and ww.any() and nw.any()             # the two classes partition the map
     assert (np.where(ww, wide, narrow) == full).all()
+
+
+def sc_wide_tensor():
+    """N1(a): ARKCOS_PLAN_WIDE_TENSOR runs the WIDE items through k_convolve_wide_tc (emulated mma.m16n8k8 TF32 with the
+    3-term split); same tolerance against the oracle, NARROW rings bit-identical to the default plan, batch entry point."""
+    w = wl.config(0)[0]
+    x32, table = w.map_f32(), w.table()
+    expect = oracle.convolve(x32, table, w.theta_cut, level=1)
+    full = convolve(x32, table, w.theta_cut)
+    tens = convolve(x32, table, w.theta_cut, flags=arkcos.PLAN_WIDE_TENSOR)
+    parity(tens, expect, what="cfg0 wide-tensor")
+    narrow_only = convolve(x32, table, w.theta_cut, flags=arkcos.PLAN_ONLY_NARROW)
+    nw = ~np.isnan(narrow_only)
+    assert nw.any() and (~nw).any()
+    assert (tens[nw] == full[nw]).all()                           # the NARROW kernel is not affected
+    assert (tens[~nw] != full[~nw]).any()                         # ... and the WIDE rings really took the other kernel
+    for n_theta, n_phi, cut_deg in [(3, 8, 61.0), (10, 20, 180.0), (20, 1028, 9.5), (7, 2052, 33.0)]:
+        rng = np.random.default_rng(n_theta * 7919 + n_phi)
+        cut = cut_deg * DEG; table = rng.standard_normal(37)
+        x = rng.standard_normal((n_theta, n_phi)).astype(np.float32)
+        got = convolve(x, table, cut, flags=arkcos.PLAN_WIDE_TENSOR)
+        parity(got, oracle.convolve(x, table, cut, level=0 if n_theta * n_phi <= 4096 else 1), what=f"wide-tensor {n_theta}x{n_phi}")
+    maps = np.stack([wl.white_map(w.n_theta, w.n_phi, s) for s in (20, 21)])
+    with arkcos.Plan(w.n_theta, w.n_phi, w.table(), w.theta_cut, flags=arkcos.PLAN_WIDE_TENSOR) as plan:
+        d_in = dev(maps); d_out = dev(maps.shape, fill=np.nan)
+        plan.convolve_batch(d_in, d_out, 2, 0)
+        for m in range(2):
+            parity(d_out[m], oracle.convolve(maps[m], w.table(), w.theta_cut, level=1), what=f"wide-tensor batch map {m}")
 
 
 SCENARIOS = {k[3:]: v for k, v in globals().items() if k.startswith("sc_")}

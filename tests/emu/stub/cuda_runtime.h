@@ -65,6 +65,10 @@ static inline unsigned char* smem_at(uint32_t addr, uint32_t bytes) {
 // accesses that go through the kernels' PTX wrappers (ld.shared reads, cp.async writes)
 void note_read(uint32_t addr, uint32_t bytes);
 static inline unsigned char* smem_read(uint32_t addr, uint32_t bytes) { unsigned char* p = smem_at(addr, bytes); note_read(addr, bytes); return p; }
+void note_store(uint32_t addr, uint32_t bytes);   // a plain st.shared: checked against earlier readers / writers, visible at once
+static inline unsigned char* smem_write(uint32_t addr, uint32_t bytes) { unsigned char* p = smem_at(addr, bytes); note_store(addr, bytes); return p; }
+// warp-level tensor-core instruction mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 (arkcos_tensor.cuh)
+void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1);
 void check_global(const void* p, size_t bytes);   // must lie inside a registered global buffer, 16-byte aligned
 // cp.async emulation: copies are queued per thread and only performed by the wait calls
 void cp_async_enqueue(uint32_t dst, const void* src);
@@ -79,4 +83,6 @@ void cp_async_wait(int keep_groups);
 static inline void __syncthreads() { emu::sync_threads(); }
 static inline void __syncwarp() { emu::sync_warp(); }
 static inline double __ldg(const double* p) { return *p; }
+static inline float __uint_as_float(uint32_t u) { float f; std::memcpy(&f, &u, 4); return f; }
+static inline uint32_t __float_as_uint(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
 static inline size_t __cvta_generic_to_shared(const void* p) { return (size_t)((const unsigned char*)p - emu::g_smem); }

@@ -19,7 +19,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 RUNNER = os.path.join(ROOT, "tests", "emu", "run_emu_api.py")
 
 SCENARIOS = ["config0", "delta_and_weights", "entry_points_bit_identical", "bad_pointers", "small_grids", "interleaved_plans",
-             "spectral", "biased_table", "class_only_flags"]
+             "spectral", "biased_table", "class_only_flags", "wide_tensor"]
 
 
 @pytest.mark.parametrize("scenario", SCENARIOS)

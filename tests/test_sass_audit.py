@@ -44,13 +44,13 @@ def opcode(line):
 
 
 def test_kernels_present_for_sm100_and_no_local_memory(sass):
-    for key in ("k_generate_weights", "k_convolve_wide", "k_convolve_narrow", "k_rfft_rings", "k_spectral_apply", "k_spectral_weights"):
+    for key in ("k_generate_weights", "k_convolve_wideE", "k_convolve_wide_tc", "k_convolve_narrow", "k_rfft_rings", "k_spectral_apply", "k_spectral_weights"):
         ops = [opcode(l) for l in find(sass, key)]
         assert not any(o.startswith(("LDL", "STL")) for o in ops), f"{key} spills to local memory"
 
 
 def test_hot_loops_are_unrolled_plain_ffma_with_cp_async_staging(sass):
-    wide = [opcode(l) for l in find(sass, "k_convolve_wide")]
+    wide = [opcode(l) for l in find(sass, "k_convolve_wideE")]
     narrow = [opcode(l) for l in find(sass, "k_convolve_narrow")]
     assert wide.count("FFMA") == 10 * 128 and narrow.count("FFMA") == 32 * 32
     assert not any(o.startswith("FFMA2") or o.startswith("HMMA") or o.startswith("UTC") for o in wide + narrow)
