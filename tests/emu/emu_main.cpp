@@ -32,12 +32,16 @@ static std::vector<T> read_file(const char* path, size_t n) {
 
 // Self-test of the hazard checker: tiny two-warp "kernels" with and without the barrier that orders a cp.async
 // write and an ld.shared read.  Modes 1 and 3 must die with EMU FAILURE (exit 3), modes 2 and 4 must pass.
+// Modes 5 and 6: barriers that can never complete (a hang on the device) must be reported as a DEADLOCK - one lane
+// waits at __syncwarp while the rest of its warp waits at __syncthreads; a lane skips a warp-collective mma.
 static int hazard_selftest(int mode) {
     static float src[8] = {1, 2, 3, 4, 5, 6, 7, 8};
     emu::g_global = {{(const unsigned char*)src, (const unsigned char*)(src + 8)}};
     emu::run_cta(0, 0, 64, 64, [&] {
         const unsigned t = threadIdx.x;
         float a, b, c, d;
+        if (mode == 5) { if (t == 3) __syncwarp(); __syncthreads(); return; }
+        if (mode == 6) { float c[4] = {0, 0, 0, 0}; if (t != 7) emu::mma_m16n8k8_tf32(c, 0, 0, 0, 0, 0, 0); return; }
         if (mode == 1 || mode == 2) {                      // write by thread 0, read by thread 40 (another warp)
             if (t == 0) { arkcos::cp_async16(0, src); arkcos::cp_async_wait_all(); }
             if (mode == 2) __syncthreads();

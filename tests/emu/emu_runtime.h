@@ -2,17 +2,24 @@
 // once per emulation binary (emu_main.cpp: the kernel-level command-line harness; emu_api.cpp: the whole C-ABI
 // library compiled for the host).
 //
-// One OS thread per CUDA thread, one CTA at a time, real barriers for __syncthreads / __syncwarp, cp.async
+// One FIBER per CUDA thread, one CTA at a time, scheduled round-robin by a single OS thread: a fiber runs
+// until it reaches __syncthreads / __syncwarp / a warp-collective instruction, where it waits until every live
+// thread of the CTA / warp has arrived (a barrier that can never complete - divergent barriers, a thread that exited
+// while its warp waits - is reported as a DEADLOCK instead of hanging).  cp.async is
 // performed only at its wait (EMU_EAGER=1: at issue), shared memory a heap block of exactly the launch's dynamic
 // size with bounds- and alignment-checked ld.shared wrappers, checked cp.async sources, NaN-initialised shared
 // memory, and a shared-memory hazard checker (the CPU counterpart of compute-sanitizer racecheck).
 #pragma once
-#include <barrier>
+#if !defined(__x86_64__)
+#include <ucontext.h>
+#endif
+
 #include <map>
 #include <memory>
-#include <mutex>
 #include <string>
-#include <thread>
+#if defined(__SANITIZE_ADDRESS__)
+#include <sanitizer/common_interface_defs.h>
+#endif
 
 #include "cuda_runtime.h"
 
@@ -22,8 +29,8 @@ dim3 g_blockDim, g_gridDim;
 unsigned char* g_smem = nullptr;
 size_t g_smem_bytes = 0;
 
-static std::unique_ptr<std::barrier<>> g_cta_barrier;
-static std::vector<std::unique_ptr<std::barrier<>>> g_warp_barriers;
+enum WaitKind { kRunnable = 0, kWaitCta = 1, kWaitWarp = 2, kWaitCollective = 3, kDone = 4 };
+static void fiber_wait(int kind);        // yield to the scheduler until the barrier of that kind completes
 struct Range { const unsigned char* lo; const unsigned char* hi; };
 static std::vector<Range> g_global;      // buffers a cp.async may read: registered by the harness, or by the emulated cudaMalloc
 
@@ -32,8 +39,8 @@ static std::vector<Range> g_global;      // buffers a cp.async may read: registe
     std::_Exit(3);
 }
 static thread_local uint32_t t_cta_epoch = 0, t_warp_epoch = 0;   // barriers this thread has passed (hazard checker below)
-void sync_threads() { g_cta_barrier->arrive_and_wait(); ++t_cta_epoch; }
-void sync_warp() { g_warp_barriers[t_threadIdx.x >> 5]->arrive_and_wait(); ++t_warp_epoch; }
+void sync_threads() { fiber_wait(kWaitCta); ++t_cta_epoch; }
+void sync_warp() { fiber_wait(kWaitWarp); ++t_warp_epoch; }
 void check_global(const void* p, size_t bytes) {
     const unsigned char* q = (const unsigned char*)p;
     if ((uintptr_t)q % 16) fail("misaligned global access of cp.async", (long)((uintptr_t)q % 16), (long)bytes);
@@ -52,7 +59,6 @@ void check_global(const void* p, size_t bytes) {
 // checked against earlier readers / writers at issue and becomes the word's writer at the wait.
 struct Stamp { uint16_t tid; uint16_t valid; uint32_t cta_epoch, warp_epoch; };
 static std::vector<Stamp> g_writer, g_reader;                     // per 4-byte word: last writer, most recent reader
-static std::mutex g_shadow_mutex;
 static const bool g_racecheck = std::getenv("EMU_NO_RACECHECK") == nullptr;
 static bool ordered_after(const Stamp& a) {                        // is the calling thread's access ordered after stamp a?
     if (!a.valid || a.tid == t_threadIdx.x) return true;
@@ -62,7 +68,6 @@ static bool ordered_after(const Stamp& a) {                        // is the cal
 static Stamp now() { return Stamp{(uint16_t)t_threadIdx.x, 1, t_cta_epoch, t_warp_epoch}; }
 void note_read(uint32_t addr, uint32_t bytes) {
     if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
     for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
         if (!ordered_after(g_writer[w])) fail("shared-memory hazard: read of a word another thread wrote without a barrier in between (word, writer)", w, g_writer[w].tid);
         const Stamp& r = g_reader[w];
@@ -71,7 +76,6 @@ void note_read(uint32_t addr, uint32_t bytes) {
 }
 static void note_write_issue(uint32_t addr, uint32_t bytes) {
     if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
     for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
         if (!ordered_after(g_reader[w])) fail("shared-memory hazard: cp.async issued into a word another thread may still be reading (word, reader)", w, g_reader[w].tid);
         if (!ordered_after(g_writer[w])) fail("shared-memory hazard: two unordered writes of one word (word, writer)", w, g_writer[w].tid);
@@ -82,7 +86,6 @@ static void note_write_issue(uint32_t addr, uint32_t bytes) {
 // barrier counts at issue.
 static void note_write_done(uint32_t addr, uint32_t bytes, uint32_t ic, uint32_t iw) {
     if (!g_racecheck) return;
-    std::lock_guard<std::mutex> lock(g_shadow_mutex);
     for (uint32_t w = addr / 4; w < (addr + bytes + 3) / 4; w++) {
         const Stamp& r = g_reader[w];
         const bool before_issue = !r.valid || r.tid == t_threadIdx.x || ic > r.cta_epoch ||
@@ -103,14 +106,18 @@ void note_store(uint32_t addr, uint32_t bytes) {                  // plain st.sh
 // t = lane & 3):  A[g + 8 (r & 1)][t + 4 (r >> 1)] = a_r,  B[t + 4 r][g] = b_r,  C[g + 8 (r >> 1)][2 t + (r & 1)] = c_r.
 // The tensor core reads the upper 19 bits of an operand register (the 13 low mantissa bits are ignored), forms
 // the products exactly and adds them to C with TRUNCATION; here: exact sum in FP64, then rounded toward zero to FP32.
-// The meeting uses the warp's barrier WITHOUT counting it for the hazard checker: mma.sync converges the warp but
+// The meeting is a warp rendezvous that is NOT counted for the hazard checker: mma.sync converges the warp but
 // orders no shared-memory access.
-static uint32_t g_mma_a[64][32][4], g_mma_b[64][32][2];
+static uint32_t g_mma_a[2][32][32][4], g_mma_b[2][32][32][2];   // [parity of the warp's mma count][warp][lane][register]
+static unsigned g_mma_count[32][32];                             // per warp and lane: mma instructions executed in this CTA
 void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
     const unsigned warp = t_threadIdx.x >> 5, lane = t_threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    uint32_t (&A)[32][4] = g_mma_a[warp]; uint32_t (&B)[32][2] = g_mma_b[warp];
+    // two exchange buffers used alternately: one rendezvous per instruction is enough, because a lane can only
+    // overwrite buffer p two instructions later, after every lane has passed the rendezvous in between
+    const unsigned par = g_mma_count[warp][lane]++ & 1u;
+    uint32_t (&A)[32][4] = g_mma_a[par][warp]; uint32_t (&B)[32][2] = g_mma_b[par][warp];
     A[lane][0] = a0; A[lane][1] = a1; A[lane][2] = a2; A[lane][3] = a3; B[lane][0] = b0; B[lane][1] = b1;
-    g_warp_barriers[warp]->arrive_and_wait();
+    fiber_wait(kWaitCollective);
     auto tf32 = [](uint32_t u) { u &= 0xFFFFE000u; float f; std::memcpy(&f, &u, 4); return (double)f; };
     for (int r = 0; r < 4; r++) {
         const unsigned m = g + 8 * (r >> 1), n = 2 * t + (r & 1);
@@ -121,7 +128,6 @@ void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint
         if (std::fabs((double)f) > std::fabs(sum)) f = std::nextafterf(f, 0.0f);
         c[r] = f;
     }
-    g_warp_barriers[warp]->arrive_and_wait();
 }
 
 struct Pending { uint32_t dst; const void* src; uint32_t ic, iw; };
@@ -155,6 +161,98 @@ static void thread_exit_check() {
     if (!t_open.empty() || !t_groups.empty()) fail("thread exits with cp.async copies it never waited for", (long)t_groups.size(), 0);
 }
 
+// ---- fibers ------------------------------------------------------------------------------------------------
+// Context switch.  glibc's swapcontext makes two system calls per switch (it saves and restores the signal mask),
+// which dominated the run time of the emulation; on x86-64 the switch is therefore a dozen instructions of our own
+// (callee-saved registers + stack pointer, System V ABI), ucontext elsewhere.
+#if defined(__x86_64__)
+extern "C" void arkcos_emu_switch(void** save_sp, void* load_sp);
+asm(".text\n.globl arkcos_emu_switch\n.type arkcos_emu_switch,@function\narkcos_emu_switch:\n"
+    "  pushq %rbp\n  pushq %rbx\n  pushq %r12\n  pushq %r13\n  pushq %r14\n  pushq %r15\n"
+    "  movq %rsp, (%rdi)\n  movq %rsi, %rsp\n"
+    "  popq %r15\n  popq %r14\n  popq %r13\n  popq %r12\n  popq %rbx\n  popq %rbp\n  ret\n"
+    ".size arkcos_emu_switch, .-arkcos_emu_switch\n");
+struct Context { void* sp = nullptr; };
+static void context_switch(Context& from, Context& to) { arkcos_emu_switch(&from.sp, to.sp); }
+static void context_make(Context& c, unsigned char* stack, size_t bytes, void (*entry)()) {
+    uintptr_t top = ((uintptr_t)stack + bytes) & ~(uintptr_t)15;
+    void** sp = (void**)top;
+    *--sp = nullptr;                       // the "return address" of entry (it never returns)
+    *--sp = (void*)entry;                  // popped by the ret of the first switch: entry starts with rsp = 8 mod 16
+    for (int r = 0; r < 6; r++) *--sp = nullptr;
+    c.sp = sp;
+}
+#else
+struct Context { ucontext_t uc; };
+static void context_switch(Context& from, Context& to) { swapcontext(&from.uc, &to.uc); }
+static void context_make(Context& c, unsigned char* stack, size_t bytes, void (*entry)()) {
+    getcontext(&c.uc);
+    c.uc.uc_stack.ss_sp = stack; c.uc.uc_stack.ss_size = bytes; c.uc.uc_link = nullptr;
+    makecontext(&c.uc, entry, 0);
+}
+#endif
+
+struct Fiber {
+    Context ctx;
+    std::unique_ptr<unsigned char[]> stack;
+    uint3 tid{0, 0, 0};
+    uint32_t cta_epoch = 0, warp_epoch = 0;
+    std::vector<std::vector<Pending>> groups;
+    std::vector<Pending> open;
+    int state = kDone;
+    void* fake_stack = nullptr;           // AddressSanitizer's bookkeeping across a switch
+};
+constexpr size_t kFiberStack = 512 * 1024;
+static std::vector<Fiber> g_fibers;
+static Fiber* g_cur = nullptr;
+static Context g_sched_ctx;
+static void* g_sched_fake_stack = nullptr;
+static const void* g_sched_stack_bottom = nullptr;
+static size_t g_sched_stack_size = 0;
+static void (*g_body)(void*) = nullptr;
+static void* g_body_arg = nullptr;
+
+static void switch_to_scheduler(bool dying) {
+    Fiber* f = g_cur;
+#if defined(__SANITIZE_ADDRESS__)
+    __sanitizer_start_switch_fiber(dying ? nullptr : &f->fake_stack, g_sched_stack_bottom, g_sched_stack_size);
+#endif
+    context_switch(f->ctx, g_sched_ctx);
+#if defined(__SANITIZE_ADDRESS__)
+    __sanitizer_finish_switch_fiber(f->fake_stack, &g_sched_stack_bottom, &g_sched_stack_size);
+#endif
+}
+static void fiber_wait(int kind) {
+    Fiber* f = g_cur;
+    f->state = kind;
+    f->cta_epoch = t_cta_epoch; f->warp_epoch = t_warp_epoch;
+    std::swap(f->groups, t_groups); std::swap(f->open, t_open);
+    switch_to_scheduler(false);
+}
+static void fiber_entry() {
+#if defined(__SANITIZE_ADDRESS__)
+    __sanitizer_finish_switch_fiber(nullptr, &g_sched_stack_bottom, &g_sched_stack_size);
+#endif
+    g_body(g_body_arg);
+    thread_exit_check();
+    g_cur->state = kDone;
+    switch_to_scheduler(true);
+}
+static void resume(Fiber& f) {
+    g_cur = &f;
+    t_threadIdx = f.tid; t_cta_epoch = f.cta_epoch; t_warp_epoch = f.warp_epoch;
+    std::swap(f.groups, t_groups); std::swap(f.open, t_open);
+    f.state = kRunnable;
+#if defined(__SANITIZE_ADDRESS__)
+    __sanitizer_start_switch_fiber(&g_sched_fake_stack, f.stack.get(), kFiberStack);
+#endif
+    context_switch(g_sched_ctx, f.ctx);
+#if defined(__SANITIZE_ADDRESS__)
+    __sanitizer_finish_switch_fiber(g_sched_fake_stack, nullptr, nullptr);
+#endif
+    g_cur = nullptr;
+}
+
 // run one CTA of `threads` threads
 template <typename F>
 static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_bytes, F&& body) {
@@ -163,18 +261,41 @@ static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_byte
     std::memset(g_smem, 0xFF, smem_bytes);                        // NaN pattern
     g_writer.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0}); g_reader.assign(smem_bytes / 4 + 4, Stamp{0, 0, 0, 0});
     g_blockDim = dim3(threads);
-    g_cta_barrier = std::make_unique<std::barrier<>>((std::ptrdiff_t)threads);
-    g_warp_barriers.clear();
-    for (unsigned w = 0; w < threads / 32; w++) g_warp_barriers.push_back(std::make_unique<std::barrier<>>(32));
-    std::vector<std::thread> pool;
-    for (unsigned t = 0; t < threads; t++)
-        pool.emplace_back([&, t] {
-            t_threadIdx = uint3{t, 0, 0}; t_blockIdx = uint3{bx, by, 0};
-            t_cta_epoch = 0; t_warp_epoch = 0;
-            body();
-            thread_exit_check();
-        });
-    for (auto& th : pool) th.join();
+    t_blockIdx = uint3{bx, by, 0};
+    std::memset(g_mma_count, 0, sizeof(g_mma_count));
+    if (g_fibers.size() < threads) g_fibers.resize(threads);
+    auto thunk = [](void* p) { (*static_cast<std::remove_reference_t<F>*>(p))(); };
+    g_body = thunk; g_body_arg = &body;
+    for (unsigned t = 0; t < threads; t++) {
+        Fiber& f = g_fibers[t];
+        if (!f.stack) f.stack.reset(new unsigned char[kFiberStack]);
+        f.tid = uint3{t, 0, 0}; f.cta_epoch = f.warp_epoch = 0; f.groups.clear(); f.open.clear(); f.state = kRunnable; f.fake_stack = nullptr;
+        context_make(f.ctx, f.stack.get(), kFiberStack, fiber_entry);
+    }
+    const unsigned warps = threads / 32;
+    for (;;) {
+        bool ran = false, all_done = true;
+        for (unsigned t = 0; t < threads; t++)
+            if (g_fibers[t].state == kRunnable) { resume(g_fibers[t]); ran = true; }
+        // barriers complete when every LIVE thread of the CTA / warp waits at the same kind of barrier
+        unsigned live = 0, at_cta = 0;
+        for (unsigned t = 0; t < threads; t++) { const int st = g_fibers[t].state; live += st != kDone; at_cta += st == kWaitCta; all_done &= st == kDone; }
+        if (all_done) break;
+        bool released = false;
+        if (live > 0 && at_cta == live) { for (unsigned t = 0; t < threads; t++) if (g_fibers[t].state == kWaitCta) g_fibers[t].state = kRunnable; released = true; }
+        for (unsigned w = 0; w < warps; w++)
+            for (const int kind : {kWaitWarp, kWaitCollective}) {
+                unsigned wl = 0, at = 0;
+                for (unsigned l = 0; l < 32; l++) { const int st = g_fibers[32 * w + l].state; wl += st != kDone; at += st == kind; }
+                if (wl > 0 && at == wl) { for (unsigned l = 0; l < 32; l++) if (g_fibers[32 * w + l].state == kind) g_fibers[32 * w + l].state = kRunnable; released = true; }
+                // a warp-collective instruction needs all 32 lanes
+                if (kind == kWaitCollective && at > 0 && at == wl && wl != 32) fail("warp-collective instruction executed by a partial warp (warp, lanes)", w, wl);
+            }
+        if (!ran && !released) {
+            for (unsigned t = 0; t < threads; t++)
+                if (g_fibers[t].state != kDone) { t_threadIdx = g_fibers[t].tid; fail("DEADLOCK: a barrier can never complete (waiting thread's barrier kind 1 = CTA, 2 = warp, 3 = collective; live threads)", g_fibers[t].state, live); }
+        }
+    }
     std::free(g_smem);
     g_smem = nullptr;
 }

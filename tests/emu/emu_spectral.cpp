@@ -1,49 +1,12 @@
 // emu_spectral.cpp - HOST EMULATION harness of the spectral-path kernels (csrc/arkcos_spectral.cuh, N2).  Test
-// infrastructure only; same stub runtime as emu_main.cpp (one OS thread per CUDA thread, real barriers, shared
-// memory a heap block of exactly the launch's size under AddressSanitizer).
+// infrastructure only; same runtime as emu_main.cpp (tests/emu/emu_runtime.h: one fiber per CUDA thread, barriers with
+// deadlock detection, shared memory a heap block of exactly the launch's size under AddressSanitizer).
 //
 //   emu_spectral n_theta n_phi theta_cut n_table table.f64 in.f32 out.f32
-#include <barrier>
-#include <memory>
-#include <thread>
-
-#include "cuda_runtime.h"
+#include "emu_runtime.h"
 
 #include "arkcos_internal.h"
 #include "arkcos_spectral.cuh"
-
-namespace emu {
-thread_local uint3 t_threadIdx, t_blockIdx;
-dim3 g_blockDim, g_gridDim;
-unsigned char* g_smem = nullptr;
-size_t g_smem_bytes = 0;
-static std::unique_ptr<std::barrier<>> g_cta_barrier;
-[[noreturn]] void fail(const char* what, long a, long b) {
-    std::fprintf(stderr, "EMU FAILURE: %s (%ld, %ld) block %u thread %u\n", what, a, b, t_blockIdx.x, t_threadIdx.x);
-    std::_Exit(3);
-}
-void sync_threads() { g_cta_barrier->arrive_and_wait(); }
-void sync_warp() {}
-void check_global(const void*, size_t) {}
-void note_read(uint32_t, uint32_t) {}
-void cp_async_enqueue(uint32_t, const void*) { fail("cp.async is not used by the spectral kernels", 0, 0); }
-void cp_async_commit_group() {}
-void cp_async_wait(int) {}
-template <typename F>
-static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_bytes, F&& body) {
-    g_smem_bytes = smem_bytes;
-    g_smem = (unsigned char*)std::malloc(smem_bytes ? smem_bytes : 16);      // exactly the launch's size: ASan sees overruns
-    std::memset(g_smem, 0xFF, smem_bytes);
-    g_blockDim = dim3(threads);
-    g_cta_barrier = std::make_unique<std::barrier<>>((std::ptrdiff_t)threads);
-    std::vector<std::thread> pool;
-    for (unsigned t = 0; t < threads; t++)
-        pool.emplace_back([&, t] { t_threadIdx = uint3{t, 0, 0}; t_blockIdx = uint3{bx, by, 0}; body(); });
-    for (auto& th : pool) th.join();
-    std::free(g_smem);
-    g_smem = nullptr;
-}
-}  // namespace emu
 
 template <typename T>
 static std::vector<T> read_file(const char* path, size_t n) {

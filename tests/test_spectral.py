@@ -23,7 +23,7 @@ DEG = math.pi / 180.0
 def emu_spectral(tmp_path_factory):
     out = str(tmp_path_factory.mktemp("emu") / "emu_spectral")
     cmd = ["g++", "-std=c++20", "-O1", "-g", "-fsanitize=address", "-fno-omit-frame-pointer", "-pthread", "-DARKCOS_HOST_EMU",
-           "-Wno-unknown-pragmas", "-I", os.path.join(EMU_DIR, "stub"), "-I", CSRC, os.path.join(EMU_DIR, "emu_spectral.cpp"),
+           "-Wno-unknown-pragmas", "-I", os.path.join(EMU_DIR, "stub"), "-I", EMU_DIR, "-I", CSRC, os.path.join(EMU_DIR, "emu_spectral.cpp"),
            os.path.join(CSRC, "arkcos_schedule.cpp"), "-o", out]
     res = subprocess.run(cmd, capture_output=True, text=True)
     assert res.returncode == 0, res.stderr[-3000:]

@@ -38,7 +38,7 @@ def check(got, x32, table, cut, max_pix=30000):
     (16, 64, 20.0, "gauss"),        # F = 1, eight tap splits (S = 8): the fragment-space reduction
     (24, 256, 9.0, "osc"),
     (9, 1500, 31.0, "osc"),         # ragged tiles (1500 = 1024 + 476), odd n_theta, several stages per row
-    (6, 4096, 50.0, "osc"),         # whole-ring windows (4096 taps = 8 stages of 512), F = 4
+    (4, 4096, 50.0, "osc"),         # whole-ring windows (4096 taps = 8 stages of 512), F = 4
     (5, 36, 179.0, "osc"),          # the input window wraps around the ring many times
 ])
 def test_emulated_tensor_wide_kernel_matches_oracle(emu_bin, tmp_path, n_theta, n_phi, cut_deg, kernel):  # noqa: F811
