@@ -37,9 +37,20 @@ static std::vector<T> read_file(const char* path, size_t n) {
 static int hazard_selftest(int mode) {
     static float src[8] = {1, 2, 3, 4, 5, 6, 7, 8};
     emu::g_global = {{(const unsigned char*)src, (const unsigned char*)(src + 8)}};
-    emu::run_cta(0, 0, 64, 64, [&] {
+    emu::g_kernel_name = "selftest";
+    emu::run_cta(0, 0, 64, mode == 7 ? 8192 : 64, [&] {
         const unsigned t = threadIdx.x;
         float a, b, c, d;
+        if (mode == 7) {                                   // bank-conflict accounting: known patterns (EMU_BANKS=<file>)
+            float a, b, c, d;
+            if (t < 32) {
+                arkcos::lds64i<0>(a, b, t * 144);          // round 1's NARROW layout: lanes l and l + 8 collide -> 2 wavefronts per half warp
+                arkcos::lds128(a, b, c, d, t * 80);        // v5's lane tiles: conflict free
+                arkcos::lds128(a, b, c, d, (t & 7) * 16);  // four lanes per address: broadcast, conflict free
+                arkcos::lds128(a, b, c, d, t * 128);       // every lane in the same four banks: 8 wavefronts per quarter warp
+            }
+            return;
+        }
         if (mode == 5) { if (t == 3) __syncwarp(); __syncthreads(); return; }
         if (mode == 6) { float c[4] = {0, 0, 0, 0}; if (t != 7) emu::mma_m16n8k8_tf32(c, 0, 0, 0, 0, 0, 0); return; }
         if (mode == 1 || mode == 2) {                      // write by thread 0, read by thread 40 (another warp)
@@ -54,6 +65,7 @@ static int hazard_selftest(int mode) {
             if (mode == 3) __syncwarp();
         }
     });
+    emu::bank_report();
     std::printf("selftest %d passed the checker\n", mode);
     return 0;
 }
@@ -92,6 +104,7 @@ int main(int argc, char** argv) {
     }
     const int gen_grid = 4;
     emu::g_gridDim = dim3(gen_grid);
+    emu::g_kernel_name = "k_generate_weights";
     for (int b = 0; b < gen_grid; b++)
         emu::run_cta((unsigned)b, 0, kGenThreads, (size_t)n_table * sizeof(double), [&] { k_generate_weights(g); });
 
@@ -113,6 +126,7 @@ int main(int argc, char** argv) {
         if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
         (wide ? n_wide : n_narrow)++;
         ConvParams cc = c;                                     // each kernel is launched on its own part of the work list
+        emu::g_kernel_name = wide ? (wide_tensor ? "k_convolve_wide_tc" : "k_convolve_wide") : "k_convolve_narrow";
         if (wide && wide_tensor) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide_tc(cc); });   // N1(a)
         else if (wide) emu::run_cta((unsigned)b, 0, kThreads, s.smem_wide, [&] { k_convolve_wide(cc); });
         else {
@@ -120,6 +134,7 @@ int main(int argc, char** argv) {
             emu::run_cta((unsigned)(b - s.n_wide_items), 0, kThreads, s.smem_narrow, [&] { k_convolve_narrow(cc); });
         }
     }
+    emu::bank_report();
     FILE* f = std::fopen(argv[7], "wb");
     if (!f || std::fwrite(out.data(), sizeof(float), n_pix, f) != n_pix) { std::fprintf(stderr, "cannot write %s\n", argv[7]); return 2; }
     std::fclose(f);

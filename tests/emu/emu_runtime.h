@@ -17,6 +17,7 @@
 #include <map>
 #include <memory>
 #include <string>
+#include <unordered_map>
 #if defined(__SANITIZE_ADDRESS__)
 #include <sanitizer/common_interface_defs.h>
 #endif
@@ -130,6 +131,77 @@ void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint
     }
 }
 
+// ---- shared-memory bank-conflict accounting (EMU_BANKS=<report file>) --------------------------------------
+// What ncu reports as l1tex__data_bank_conflicts_pipe_lsu_mem_shared, from the addresses the emulation sees: the
+// accesses of the 32 lanes of a warp that belong to one executed instruction are matched by (warp, barrier counts,
+// call site = the instruction's address in the emulation binary, occurrence of that site since the last barrier);
+// shared memory has 32 banks of 4 bytes, a 16-byte access is served a quarter warp at a time, an 8-byte access a
+// half warp, and a phase takes as many wavefronts as the largest number of DIFFERENT words it touches in one bank
+// (equal words are a broadcast).  Report per (kernel, site): instructions, wavefronts, conflict-free wavefronts.
+bool g_banks = std::getenv("EMU_BANKS") != nullptr;
+const char* g_kernel_name = "?";
+struct BankKey {
+    uint32_t warp, ce, we, occ; uintptr_t site;
+    bool operator==(const BankKey& o) const { return warp == o.warp && ce == o.ce && we == o.we && occ == o.occ && site == o.site; }
+};
+struct BankKeyHash { size_t operator()(const BankKey& k) const { return std::hash<uint64_t>()(((uint64_t)k.warp << 48) ^ ((uint64_t)k.ce << 40) ^ ((uint64_t)k.we << 20) ^ k.occ ^ (k.site * 0x9E3779B97F4A7C15ull)); } };
+struct BankEntry { uint32_t addr[32]; uint32_t mask = 0; uint8_t bytes = 0, kind = 0; };
+struct SiteStat { unsigned long long instrs = 0, waves = 0, ideal = 0; unsigned worst = 0; unsigned bytes = 0, kind = 0; };
+static std::unordered_map<BankKey, BankEntry, BankKeyHash> g_bank_entries;                 // of the running CTA
+static std::map<std::pair<std::string, uintptr_t>, SiteStat> g_site_stats;                // of the whole run
+struct Occurrences { uint32_t ce = ~0u, we = ~0u; std::unordered_map<uintptr_t, uint32_t> count; };
+static std::vector<Occurrences> g_occ;                                                     // per thread of the CTA
+__attribute__((noinline)) void bank_note(uint32_t addr, uint32_t bytes, int kind) {
+    const uintptr_t site = (uintptr_t)__builtin_return_address(0);
+    const unsigned tid = t_threadIdx.x;
+    if (g_occ.size() <= tid) g_occ.resize(tid + 1);
+    Occurrences& oc = g_occ[tid];
+    if (oc.ce != t_cta_epoch || oc.we != t_warp_epoch) { oc.ce = t_cta_epoch; oc.we = t_warp_epoch; oc.count.clear(); }
+    const uint32_t occ = oc.count[site]++;
+    BankEntry& e = g_bank_entries[BankKey{tid >> 5, t_cta_epoch, t_warp_epoch, occ, site}];
+    e.addr[tid & 31] = addr; e.mask |= 1u << (tid & 31); e.bytes = (uint8_t)bytes; e.kind = (uint8_t)kind;
+}
+static void bank_finish_cta() {
+    for (auto& kv : g_bank_entries) {
+        const BankEntry& e = kv.second;
+        const unsigned lanes_per_phase = e.bytes >= 16 ? 8 : e.bytes == 8 ? 16 : 32, words = e.bytes / 4 ? e.bytes / 4 : 1;
+        unsigned waves = 0, ideal = 0;
+        for (unsigned l0 = 0; l0 < 32; l0 += lanes_per_phase) {
+            std::vector<uint32_t> per_bank[32];
+            bool any = false;
+            for (unsigned l = l0; l < l0 + lanes_per_phase; l++) {
+                if (!(e.mask >> l & 1u)) continue;
+                any = true;
+                for (unsigned j = 0; j < words; j++) {
+                    const uint32_t word = e.addr[l] / 4 + j;
+                    auto& v = per_bank[word & 31];
+                    if (std::find(v.begin(), v.end(), word) == v.end()) v.push_back(word);
+                }
+            }
+            if (!any) continue;
+            unsigned worst = 1;
+            for (auto& v : per_bank) worst = std::max<unsigned>(worst, (unsigned)v.size());
+            waves += worst; ideal += 1;
+        }
+        SiteStat& st = g_site_stats[{g_kernel_name, kv.first.site}];
+        st.instrs++; st.waves += waves; st.ideal += ideal; st.worst = std::max(st.worst, ideal ? (waves + ideal - 1) / ideal : 0u);
+        st.bytes = e.bytes; st.kind = e.kind;
+    }
+    g_bank_entries.clear();
+    g_occ.clear();
+}
+// one line per (kernel, instruction site): kernel kind bytes instructions wavefronts conflict-free-wavefronts worst-factor
+static void bank_report() {
+    const char* path = std::getenv("EMU_BANKS");
+    if (!path) return;
+    FILE* f = std::fopen(path, "w");
+    if (!f) return;
+    for (auto& kv : g_site_stats)
+        std::fprintf(f, "%s %s %u %llu %llu %llu %u\n", kv.first.first.c_str(), kv.second.kind == 0 ? "ld.shared" : kv.second.kind == 1 ? "st.shared" : "cp.async",
+                     kv.second.bytes, kv.second.instrs, kv.second.waves, kv.second.ideal, kv.second.worst);
+    std::fclose(f);
+}
+
 struct Pending { uint32_t dst; const void* src; uint32_t ic, iw; };
 static thread_local std::vector<std::vector<Pending>> t_groups;   // committed groups, oldest first
 static thread_local std::vector<Pending> t_open;                  // not yet committed
@@ -138,6 +210,16 @@ static thread_local std::vector<Pending> t_open;                  // not yet com
 // copy into a buffer that other threads still read clobbers it (WAR hazard).
 static const bool g_eager = std::getenv("EMU_EAGER") != nullptr;
 void cp_async_enqueue(uint32_t dst, const void* src) {
+    if (g_banks) {                                       // the destination side of the LDGSTS; site = the caller's instruction
+        const uintptr_t site = (uintptr_t)__builtin_return_address(0);
+        const unsigned tid = t_threadIdx.x;
+        if (g_occ.size() <= tid) g_occ.resize(tid + 1);
+        Occurrences& oc = g_occ[tid];
+        if (oc.ce != t_cta_epoch || oc.we != t_warp_epoch) { oc.ce = t_cta_epoch; oc.we = t_warp_epoch; oc.count.clear(); }
+        const uint32_t occ = oc.count[site]++;
+        BankEntry& e = g_bank_entries[BankKey{tid >> 5, t_cta_epoch, t_warp_epoch, occ, site}];
+        e.addr[tid & 31] = dst; e.mask |= 1u << (tid & 31); e.bytes = 16; e.kind = 2;
+    }
     (void)smem_at(dst, 16);
     check_global(src, 16);
     note_write_issue(dst, 16);
@@ -296,6 +378,7 @@ static void run_cta(unsigned bx, unsigned by, unsigned threads, size_t smem_byte
                 if (g_fibers[t].state != kDone) { t_threadIdx = g_fibers[t].tid; fail("DEADLOCK: a barrier can never complete (waiting thread's barrier kind 1 = CTA, 2 = warp, 3 = collective; live threads)", g_fibers[t].state, live); }
         }
     }
+    if (g_banks) bank_finish_cta();
     std::free(g_smem);
     g_smem = nullptr;
 }

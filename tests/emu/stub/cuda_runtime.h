@@ -64,14 +64,25 @@ static inline unsigned char* smem_at(uint32_t addr, uint32_t bytes) {
 // shared-memory hazard checker (emu_main.cpp): the CPU counterpart of `compute-sanitizer --tool racecheck` for the
 // accesses that go through the kernels' PTX wrappers (ld.shared reads, cp.async writes)
 void note_read(uint32_t addr, uint32_t bytes);
-static inline unsigned char* smem_read(uint32_t addr, uint32_t bytes) { unsigned char* p = smem_at(addr, bytes); note_read(addr, bytes); return p; }
+// bank-conflict accounting (EMU_BANKS=<report file>; emu_runtime.h): the call site identifies the instruction
+extern bool g_banks;
+void bank_note(uint32_t addr, uint32_t bytes, int kind);   // kind: 0 = ld.shared, 1 = st.shared, 2 = cp.async destination
+static inline __attribute__((always_inline)) unsigned char* smem_read(uint32_t addr, uint32_t bytes) {
+    unsigned char* p = smem_at(addr, bytes); note_read(addr, bytes);
+    if (g_banks) bank_note(addr, bytes, 0);
+    return p;
+}
 void note_store(uint32_t addr, uint32_t bytes);   // a plain st.shared: checked against earlier readers / writers, visible at once
-static inline unsigned char* smem_write(uint32_t addr, uint32_t bytes) { unsigned char* p = smem_at(addr, bytes); note_store(addr, bytes); return p; }
+static inline __attribute__((always_inline)) unsigned char* smem_write(uint32_t addr, uint32_t bytes) {
+    unsigned char* p = smem_at(addr, bytes); note_store(addr, bytes);
+    if (g_banks) bank_note(addr, bytes, 1);
+    return p;
+}
 // warp-level tensor-core instruction mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 (arkcos_tensor.cuh)
 void mma_m16n8k8_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1);
 void check_global(const void* p, size_t bytes);   // must lie inside a registered global buffer, 16-byte aligned
 // cp.async emulation: copies are queued per thread and only performed by the wait calls
-void cp_async_enqueue(uint32_t dst, const void* src);
+void cp_async_enqueue(uint32_t dst, const void* src) __attribute__((noinline));
 void cp_async_commit_group();
 void cp_async_wait(int keep_groups);
 }  // namespace emu
