@@ -22,10 +22,9 @@ CSRC = os.path.join(ROOT, "paper_1211_3556_b200", "csrc")
 EMU_BIN = os.path.join(EMU_DIR, "emu_arkcos")
 
 
-@pytest.fixture(scope="module")
-def emu_bin():
+def build_emu_binary():
     srcs = [os.path.join(EMU_DIR, "emu_main.cpp"), os.path.join(CSRC, "arkcos_schedule.cpp")]
-    deps = srcs + [os.path.join(CSRC, "arkcos_kernels.cuh"), os.path.join(CSRC, "arkcos_internal.h"),
+    deps = srcs + [os.path.join(CSRC, "arkcos_kernels.cuh"), os.path.join(CSRC, "arkcos_tensor.cuh"), os.path.join(CSRC, "arkcos_internal.h"),
                    os.path.join(EMU_DIR, "stub", "cuda_runtime.h"), os.path.join(EMU_DIR, "emu_runtime.h")]
     if not os.path.exists(EMU_BIN) or any(os.path.getmtime(d) > os.path.getmtime(EMU_BIN) for d in deps):
         cmd = ["g++", "-std=c++20", "-O1", "-g", "-fsanitize=address", "-fno-omit-frame-pointer", "-pthread",
@@ -33,6 +32,11 @@ def emu_bin():
         res = subprocess.run(cmd, capture_output=True, text=True)
         assert res.returncode == 0, res.stderr[-3000:]
     return EMU_BIN
+
+
+@pytest.fixture(scope="module")
+def emu_bin():
+    return build_emu_binary()
 
 
 def emulate(emu, tmp_path, x32, table, theta_cut, only=None, env=None):
