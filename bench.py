@@ -172,7 +172,7 @@ def workload_config(w: wl.Workload):
 
 
 def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want_cpu: bool, want_e2e: bool = True,
-            only: str = "all", path: str = "direct", wide_tensor: bool = False):
+            only: str = "all", path: str = "direct", wide_tensor: bool = False, all_wide: bool = False):
     """One step = S2 + S3 over ALL maps of the workload (configs[4]: the batch of 8 through arkcos_convolve_batch).
     path = "spectral": the N2 cross-check path (arkcos_convolve_spectral) instead; its step has no S2 (the weight
     spectra are plan-time) and is timed as a whole."""
@@ -193,6 +193,8 @@ def measure(w: wl.Workload, steps: int, warmup: int, dist, local_rank: int, want
         flags |= arkcos.PLAN_SPECTRAL
     if wide_tensor:                                     # N1(a) experiment: WIDE items through k_convolve_wide_tc
         flags |= arkcos.PLAN_WIDE_TENSOR
+    if all_wide:                                        # measurement hook: no NARROW class at all
+        flags |= arkcos.PLAN_ALL_WIDE
     plan = arkcos.Plan(w.n_theta, w.n_phi, table, w.theta_cut, flags=flags)
     info = plan.info()
     stream = torch.cuda.Stream(device=dev)
@@ -357,6 +359,9 @@ def main():
     ap.add_argument("--wide-tensor", action="store_true",
                     help="N1(a) experiment: the WIDE work items on the tensor cores (mma.m16n8k8 TF32, 3-term split; "
                          "ARKCOS_PLAN_WIDE_TENSOR) instead of the default FFMA kernel; the line says so in config.wide_path")
+    ap.add_argument("--all-wide", action="store_true",
+                    help="measurement hook: every ring in the WIDE class (ARKCOS_PLAN_ALL_WIDE), to compare the NARROW kernel "
+                         "with the WIDE kernel (FFMA, or tensor cores with --wide-tensor) on the same rings")
     ap.add_argument("--only", default="all", choices=["all", "wide", "narrow"],
                     help="measurement hook: launch only the WIDE or only the NARROW work items (partial output; "
                          "prints a per-class line, not the bench line)")
@@ -381,7 +386,7 @@ def main():
     if args.only != "all":
         if rank == 0:
             res = measure(w, args.steps, args.warmup, None, local_rank, want_cpu=False, want_e2e=False, only=args.only,
-                          wide_tensor=args.wide_tensor)
+                          wide_tensor=args.wide_tensor, all_wide=args.all_wide)
             info = res["info"]
             slots = int(info.fma_slots_wide) if args.only == "wide" else int(info.fma_slots) - int(info.fma_slots_wide)
             slots *= res["n_maps"]
@@ -394,7 +399,8 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, path=args.path, wide_tensor=args.wide_tensor)
+    res = measure(w, args.steps, args.warmup, dist, local_rank, want_cpu=False, path=args.path, wide_tensor=args.wide_tensor,
+                  all_wide=args.all_wide)
     units = float(res["info"].pair_evals) * res["n_maps"] * args.steps
     total_ms, total_units = replicas.aggregate(dist, res["elapsed_ms"], units, device=dev)
     if rank == 0:
@@ -402,6 +408,8 @@ def main():
         line = build_line(w, args, res, world, total_ms, total_units, cpu)
         if args.path == "spectral":
             spectral_line(line, w, res)
+        if args.all_wide:
+            line["config"]["ring_classes"] = "all rings WIDE (measurement hook ARKCOS_PLAN_ALL_WIDE, not the default schedule)"
         if args.wide_tensor:
             line["config"]["wide_path"] = "tensor cores: k_convolve_wide_tc, mma.m16n8k8 TF32 x 3-term split (N1(a) experiment, not the default)"
             line["roofline"]["kernel"] = "k_convolve_wide_tc + k_convolve_narrow"

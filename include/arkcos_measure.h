@@ -26,6 +26,11 @@ extern "C" {
  * meets the same tolerance against the oracle.  The NARROW items are not affected. */
 #define ARKCOS_PLAN_WIDE_TENSOR 32u
 
+/* Flag of arkcos_plan_create_ex: the scheduler puts EVERY ring into the WIDE class (no band marching), so that the
+ * NARROW kernel can be measured against the WIDE kernel - FFMA or, with ARKCOS_PLAN_WIDE_TENSOR, tensor cores - on
+ * the same rings.  A complete, correct convolution (the same sum in another order); only slower or faster. */
+#define ARKCOS_PLAN_ALL_WIDE 64u
+
 /*
  * arkcos_measure_convolve - one arkcos_convolve_batch on `stream` with CUDA events (created and destroyed
  * inside the call) around each kernel; synchronises the stream and returns the device time of the weight

@@ -19,6 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, EINTERNAL = 0, 1, 2, 3, 4, 5
 PLAN_DEFAULT, PLAN_HOST_ONLY, PLAN_CACHE_WEIGHTS = 0, 1, 2
 PLAN_ONLY_WIDE, PLAN_ONLY_NARROW = 4, 8      # measurement hooks (include/arkcos_measure.h)
 PLAN_WIDE_TENSOR = 32                        # N1(a) experiment: WIDE items on the tensor cores (include/arkcos_measure.h)
+PLAN_ALL_WIDE = 64                           # measurement hook: every ring in the WIDE class (include/arkcos_measure.h)
 PLAN_SPECTRAL = 16                           # N2, the phi-spectral ring-pair path (include/arkcos_spectral.h)
 
 _c_plan_p = ctypes.c_void_p

@@ -265,7 +265,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
     if (!k_table || n_table < 2 || n_theta < 1 || n_phi < 1) return ARKCOS_EINVAL;
     if (!(theta_cut > 0.0) || !std::isfinite(theta_cut)) return ARKCOS_EINVAL;
     if (flags & ~(ARKCOS_PLAN_HOST_ONLY | ARKCOS_PLAN_CACHE_WEIGHTS | ARKCOS_PLAN_ONLY_WIDE | ARKCOS_PLAN_ONLY_NARROW | ARKCOS_PLAN_SPECTRAL |
-                  ARKCOS_PLAN_WIDE_TENSOR)) return ARKCOS_EINVAL;
+                  ARKCOS_PLAN_WIDE_TENSOR | ARKCOS_PLAN_ALL_WIDE)) return ARKCOS_EINVAL;
     if ((flags & ARKCOS_PLAN_SPECTRAL) && (n_phi < 16 || n_phi > kSpecMaxPhi || (n_phi & (n_phi - 1)) != 0)) return ARKCOS_EUNSUPPORTED;
     if ((flags & ARKCOS_PLAN_ONLY_WIDE) && (flags & ARKCOS_PLAN_ONLY_NARROW)) return ARKCOS_EINVAL;
     for (int m = 0; m < n_table; m++) if (!std::isfinite(k_table[m])) return ARKCOS_EINVAL;
@@ -285,7 +285,7 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan** plan, int n_theta, int n_p
             pl->sm_count = prop.multiProcessorCount;
             if (prop.major < 10) { g_last_cuda_error = "arkcos needs an sm_100 class device"; delete pl; return ARKCOS_EUNSUPPORTED; }
         }
-        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched);
+        int rc = build_schedule(n_theta, n_phi, theta_cut, pl->sm_count, pl->sched, (flags & ARKCOS_PLAN_ALL_WIDE) != 0);
         if (rc != 0) { delete pl; return (arkcos_status)rc; }
     } catch (const std::bad_alloc&) { delete pl; return ARKCOS_ENOMEM; }
     if (flags & ARKCOS_PLAN_HOST_ONLY) { *plan = pl; return ARKCOS_OK; }

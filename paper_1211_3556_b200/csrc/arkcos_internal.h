@@ -162,7 +162,9 @@ size_t wide_smem_bytes(int R);
 size_t narrow_smem_bytes(int R, int wcap);
 
 // Builds the schedule.  Returns 0 on success, 1 = invalid argument, 4 = unsupported (matches arkcos_status).
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out);
+// all_wide: every ring goes to the WIDE class (measurement hook ARKCOS_PLAN_ALL_WIDE: the NARROW kernel against the
+// WIDE kernel on the same rings).
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& out, bool all_wide = false);
 
 // Re-derives, as plain integer arithmetic, every global-memory range and every shared-memory offset the
 // kernels will form from the schedule's descriptors (work items, pair descriptors, narrow runs, generator

@@ -46,7 +46,7 @@ int Schedule::window(int i, int j) const {
     return window_of(*this, i, j);
 }
 
-int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s) {
+int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Schedule& s, bool all_wide) {
     if (n_theta < 1 || n_phi < 4 || !(theta_cut > 0.0) || !(theta_cut <= kPi * (1.0 + 1e-15))) return 1;
     if (n_phi % 4 != 0) return 4;
     if (sm_count < 1) sm_count = 148;
@@ -118,7 +118,7 @@ int build_schedule(int n_theta, int n_phi, double theta_cut, int sm_count, Sched
         return true;
     };
     s.first_narrow = s.n_north;
-    while (s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
+    while (!all_wide && s.first_narrow > 0 && ring_is_narrow(s.first_narrow - 1)) s.first_narrow--;
     // stored windows of the narrow rings
     std::vector<int> nw_start((size_t)s.n_north * W, 0), nw_ntaps((size_t)s.n_north * W, 0);
     for (int i = s.first_narrow; i < s.n_north; i++)

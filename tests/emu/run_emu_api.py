@@ -273,6 +273,11 @@ def sc_wide_tensor():
         x = rng.standard_normal((n_theta, n_phi)).astype(np.float32)
         got = convolve(x, table, cut, flags=arkcos.PLAN_WIDE_TENSOR)
         parity(got, oracle.convolve(x, table, cut, level=0 if n_theta * n_phi <= 4096 else 1), what=f"wide-tensor {n_theta}x{n_phi}")
+    # every ring WIDE (measurement hook), FFMA and tensor
+    for fl in (arkcos.PLAN_ALL_WIDE, arkcos.PLAN_ALL_WIDE | arkcos.PLAN_WIDE_TENSOR):
+        with arkcos.Plan(w.n_theta, w.n_phi, w.table(), w.theta_cut, flags=fl | arkcos.PLAN_HOST_ONLY) as hp:
+            assert hp.info().first_narrow_ring == (w.n_theta + 1) // 2 and hp.validate()[0] == 0
+        parity(convolve(x32, w.table(), w.theta_cut, flags=fl), expect, what=f"cfg0 all-wide flags {fl}")
     maps = np.stack([wl.white_map(w.n_theta, w.n_phi, s) for s in (20, 21)])
     with arkcos.Plan(w.n_theta, w.n_phi, w.table(), w.theta_cut, flags=arkcos.PLAN_WIDE_TENSOR) as plan:
         d_in = dev(maps); d_out = dev(maps.shape, fill=np.nan)

@@ -48,7 +48,7 @@ def test_argument_validation():
             arkcos.Plan(nt, nph, tab, cut, flags=arkcos.PLAN_HOST_ONLY)
         assert e.value.status == status, (nt, nph, cut)
     with pytest.raises(arkcos.ArkcosError) as e:
-        arkcos.Plan(4, 8, t, 0.5, flags=64)
+        arkcos.Plan(4, 8, t, 0.5, flags=1024)
     assert e.value.status == arkcos.EINVAL
 
 
