@@ -117,12 +117,14 @@ int main(int argc, char** argv) {
     emu::g_global.push_back({(const unsigned char*)s.runs.data(), (const unsigned char*)(s.runs.data() + s.runs.size())});
     emu::g_gridDim = dim3((unsigned)s.items.size());
     int n_wide = 0, n_narrow = 0;
-    // EMU_ITEM_STRIDE=n: run every n-th work item only (big grids; outputs of the skipped items stay NaN)
+    // EMU_ITEM_STRIDE=n: run every n-th work item only (big grids; outputs of the skipped items stay NaN);
+    // EMU_ITEM_OFFSET=o: ... the items o, o + n, o + 2n, ... (n processes with o = 0 .. n-1 cover the launch)
     const size_t item_stride = std::getenv("EMU_ITEM_STRIDE") ? (size_t)std::atoi(std::getenv("EMU_ITEM_STRIDE")) : 1;
+    const size_t item_offset = std::getenv("EMU_ITEM_OFFSET") ? (size_t)std::atoi(std::getenv("EMU_ITEM_OFFSET")) : 0;   // items b = offset mod stride
     const bool wide_tensor = std::getenv("EMU_WIDE_TENSOR") != nullptr;   // WIDE items through k_convolve_wide_tc
     for (size_t b = 0; b < s.items.size(); b++) {
         const bool wide = s.items[b].kind == kWide;
-        if (item_stride > 1 && b % item_stride != 0) continue;
+        if (item_stride > 1 && b % item_stride != item_offset % item_stride) continue;
         if ((only == "only_wide" && !wide) || (only == "only_narrow" && wide)) continue;
         (wide ? n_wide : n_narrow)++;
         ConvParams cc = c;                                     // each kernel is launched on its own part of the work list

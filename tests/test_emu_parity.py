@@ -199,6 +199,34 @@ def test_emulated_subsets_of_the_full_size_schedules(emu_bin, tmp_path, cfg, k, 
     assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
 
 
+def test_emulated_config1_whole_map(emu_bin, tmp_path):
+    """BASELINE configs[1] (1024 x 2048, FWHM 30', 8.95e8 kernel-pixel evaluations) COMPLETE: every work item of the
+    launch through the emulated generator and both convolution kernels, the whole map against the oracle and the
+    committed golden samples - the same assertions tests/test_gpu_parity.py::test_config1_full_map_and_golden makes on
+    the device."""
+    from paper_1211_3556_b200 import workloads as wl
+    from tests.test_golden import load_golden
+    w = wl.config(1)[0]
+    x32, table = w.map_f32(), w.table()
+    from concurrent.futures import ThreadPoolExecutor
+    parts = 4                                  # four emulation processes, each every 4th work item of the launch
+    dirs = [tmp_path / f"part{o}" for o in range(parts)]
+    for d in dirs:
+        d.mkdir()
+    with ThreadPoolExecutor(parts) as ex:
+        outs = list(ex.map(lambda o: emulate(emu_bin, dirs[o], x32, table, w.theta_cut,
+                                             env={"EMU_ITEM_STRIDE": str(parts), "EMU_ITEM_OFFSET": str(o)})[0], range(parts)))
+    written = np.stack([~np.isnan(o) for o in outs])
+    assert (written.sum(axis=0) == 1).all()    # every output pixel written by exactly one work item
+    got = np.nansum(np.stack(outs), axis=0)
+    expect = oracle.convolve(x32, table, w.theta_cut, level=1)
+    rms = math.sqrt((expect ** 2).mean())
+    err = got - expect
+    assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5
+    pix, gold = load_golden("cfg1_samples.txt")
+    assert float(np.abs(got.reshape(-1)[pix] - gold).max()) / rms <= 1e-5
+
+
 @pytest.mark.parametrize("mode,must_fail", [(1, True), (2, False), (3, True), (4, False), (5, True), (6, True)])
 def test_emulation_hazard_checker_catches_missing_barriers(emu_bin, mode, must_fail):
     """The emulation's shared-memory hazard checker (the CPU counterpart of compute-sanitizer racecheck for cp.async
