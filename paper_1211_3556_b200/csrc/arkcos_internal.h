@@ -54,6 +54,8 @@ constexpr int kWideZChunks = (kWarpSpan + kWideStage) / 4 + 8;          // logic
 constexpr int kWideZBytes = (kWideZChunks + kWideZChunks / 8 + 1) * 16; // ... in the padded tile layout
 constexpr int kWideWBytes = (kWideStage + 8) * 4;   // weights of a stage (+ prefetch slack)
 constexpr int kWideStageBytes = kWideZBytes + kWideWBytes;
+constexpr int kWideFlushSteps = 128;                // blocked summation: flush the register accumulators every >= 512 taps (one full stage)
+constexpr int kWidePartBytes = kWarps * kLaneP * 32 * 4;   // per-lane partial sums of the blocked summation, [warp][output][lane]
 
 // One (north output ring i, input ring j = i + r) pair.  The southern mirror pair
 // (n_theta-1-i, n_theta-1-j) has identical weights.  `ntaps` FP32 weights w[e], tap e <-> dphi index

@@ -446,7 +446,7 @@ void build_pipeline(const Schedule& s, int n_chunks, Pipeline& p) {
 }
 
 size_t wide_smem_bytes(int R) {
-    const size_t stage = (size_t)kWarps * 2 * kWideStageBytes + (size_t)(2 * R + 1) * sizeof(PairDesc);
+    const size_t stage = (size_t)kWarps * 2 * kWideStageBytes + (size_t)(2 * R + 1) * sizeof(PairDesc) + (size_t)kWidePartBytes;
     const size_t red = (size_t)kWarps * kWarpSpan * 4;
     return stage > red ? stage : red;
 }

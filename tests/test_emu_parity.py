@@ -39,13 +39,13 @@ def emu_bin():
     return build_emu_binary()
 
 
-def emulate(emu, tmp_path, x32, table, theta_cut, only=None, env=None):
+def emulate(emu, tmp_path, x32, table, theta_cut, only=None, env=None, timeout=600):
     n_theta, n_phi = x32.shape
     t, i, o = (str(tmp_path / n) for n in ("table.f64", "in.f32", "out.f32"))
     np.ascontiguousarray(table, dtype=np.float64).tofile(t)
     np.ascontiguousarray(x32, dtype=np.float32).tofile(i)
     cmd = [emu, str(n_theta), str(n_phi), repr(float(theta_cut)), str(table.size), t, i, o] + ([only] if only else [])
-    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=dict(os.environ, **(env or {})))
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, env=dict(os.environ, **(env or {})))
     assert res.returncode == 0, (res.stdout + res.stderr)[-3000:]
     return np.fromfile(o, dtype=np.float32).reshape(n_theta, n_phi).astype(np.float64), res.stdout
 
@@ -199,6 +199,27 @@ def test_emulated_subsets_of_the_full_size_schedules(emu_bin, tmp_path, cfg, k, 
     assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5, log
 
 
+def emulate_whole_launch(emu_bin, tmp_path, w, parts):
+    """Every work item of the launch in `parts` concurrent emulation processes (each takes every parts-th item);
+    returns the merged map after checking that every output pixel was written by exactly one work item."""
+    from concurrent.futures import ThreadPoolExecutor
+    x32, table = w.map_f32(), w.table()
+    dirs = [tmp_path / f"part{o}" for o in range(parts)]
+    for d in dirs:
+        d.mkdir()
+    with ThreadPoolExecutor(parts) as ex:
+        outs = list(ex.map(lambda o: emulate(emu_bin, dirs[o], x32, table, w.theta_cut,
+                                             env={"EMU_ITEM_STRIDE": str(parts), "EMU_ITEM_OFFSET": str(o)})[0].astype(np.float32), range(parts)))
+    count = np.zeros(x32.shape, dtype=np.int32)
+    got = np.zeros(x32.shape, dtype=np.float64)
+    for o in outs:
+        wr = ~np.isnan(o)
+        count += wr
+        got[wr] += o[wr]
+    assert (count == 1).all()
+    return got
+
+
 def test_emulated_config1_whole_map(emu_bin, tmp_path):
     """BASELINE configs[1] (1024 x 2048, FWHM 30', 8.95e8 kernel-pixel evaluations) COMPLETE: every work item of the
     launch through the emulated generator and both convolution kernels, the whole map against the oracle and the
@@ -207,24 +228,28 @@ def test_emulated_config1_whole_map(emu_bin, tmp_path):
     from paper_1211_3556_b200 import workloads as wl
     from tests.test_golden import load_golden
     w = wl.config(1)[0]
-    x32, table = w.map_f32(), w.table()
-    from concurrent.futures import ThreadPoolExecutor
-    parts = 4                                  # four emulation processes, each every 4th work item of the launch
-    dirs = [tmp_path / f"part{o}" for o in range(parts)]
-    for d in dirs:
-        d.mkdir()
-    with ThreadPoolExecutor(parts) as ex:
-        outs = list(ex.map(lambda o: emulate(emu_bin, dirs[o], x32, table, w.theta_cut,
-                                             env={"EMU_ITEM_STRIDE": str(parts), "EMU_ITEM_OFFSET": str(o)})[0], range(parts)))
-    written = np.stack([~np.isnan(o) for o in outs])
-    assert (written.sum(axis=0) == 1).all()    # every output pixel written by exactly one work item
-    got = np.nansum(np.stack(outs), axis=0)
-    expect = oracle.convolve(x32, table, w.theta_cut, level=1)
+    got = emulate_whole_launch(emu_bin, tmp_path, w, 4)
+    expect = oracle.convolve(w.map_f32(), w.table(), w.theta_cut, level=1)
     rms = math.sqrt((expect ** 2).mean())
     err = got - expect
     assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5
     pix, gold = load_golden("cfg1_samples.txt")
     assert float(np.abs(got.reshape(-1)[pix] - gold).max()) / rms <= 1e-5
+
+
+def test_emulated_config2_planck_whole_map(emu_bin, tmp_path):
+    """BASELINE configs[2], the Planck-resolution workload north_star's target is quoted on (4096 x 8192, 1.73e10
+    kernel-pixel evaluations), COMPLETE: all 1610 work items of the launch bench.py times, in 8 emulation processes;
+    60 000 evenly spaced pixels and the two polar rings against the oracle.  (tests/emu/deep_audit.py does the same for
+    every BASELINE workload; profiles/r2_emulation_deep_audit.txt.)"""
+    from paper_1211_3556_b200 import workloads as wl
+    w = wl.config(2)[0]
+    got = emulate_whole_launch(emu_bin, tmp_path, w, 8)
+    pix = np.unique(np.concatenate([np.arange(0, w.n_pix, w.n_pix // 60000), np.arange(0, w.n_phi, 8), (w.n_theta - 1) * w.n_phi + np.arange(3, w.n_phi, 8)]))
+    expect = oracle.convolve(w.map_f32(), w.table(), w.theta_cut, level=1, pixels=pix)
+    rms = math.sqrt((got ** 2).mean())
+    err = got.reshape(-1)[pix] - expect
+    assert math.sqrt((err ** 2).mean()) / rms <= 1e-6 and float(np.abs(err).max()) / rms <= 1e-5
 
 
 @pytest.mark.parametrize("mode,must_fail", [(1, True), (2, False), (3, True), (4, False), (5, True), (6, True)])
