@@ -182,6 +182,11 @@ __device__ void conv_wide_tc(const ConvParams& p, const Item& it, char* smem, co
     float acc[kLaneP];
 #pragma unroll
     for (int m = 0; m < kLaneP; m++) acc[m] = 0.f;
+    // blocked summation as in conv_wide: the FP32 accumulators (one FADD per 16 taps) are flushed to per-lane partial
+    // sums in shared memory after every full stage, so a chain is ~32 additions long whatever the ring band
+    float* part = reinterpret_cast<float*>(smem + (size_t)kWarps * 2 * kWideStageBytes + (size_t)W * sizeof(PairDesc)) + warp * kLaneP * 32 + lane;
+    int since = 0;
+    bool flushed = false;
 
     WideStage cur, nxt;
     bool have = next_stage(cur);
@@ -194,7 +199,22 @@ __device__ void conv_wide_tc(const ConvParams& p, const Item& it, char* smem, co
         const uint32_t zb = woff0 + (uint32_t)(b * kWideStageBytes);
         tc_taps(acc, smem, zb, zb + (uint32_t)kTcZBytes, cur.nq, lane);
         __syncwarp();
+        since += cur.nq;
+        if (more && since >= kWideFlushSteps) {                // warp uniform; every lane touches its own words only
+#pragma unroll
+            for (int m = 0; m < kLaneP; m++) {
+                float v = acc[m];
+                if (flushed) v += part[m * 32];
+                part[m * 32] = v;
+                acc[m] = 0.f;
+            }
+            flushed = true; since = 0;
+        }
         cur = nxt; have = more; b ^= 1;
+    }
+    if (flushed) {
+#pragma unroll
+        for (int m = 0; m < kLaneP; m++) acc[m] += part[m * 32];
     }
 
     // ---- epilogue: acc[4 nt + c] is output K0 + 128 nt + 32 t + 16 (c & 1) + 8 (c >> 1) + g --------------------

@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 # 8th part of the launch runs and "exactly once" becomes "at most once")
 RUNS = [(1, 0, False), (2, 0, False), (3, 0, False), (3, 1, False), (3, 2, False), (3, 3, False),
         (4, 0, False), (4, 1, False), (4, 2, False), (4, 3, False), (2, 0, True), (3, 3, True), (4, 3, True), (9, 0, False), (9, 0, True)]
-PAPER_PARTS = 64          # the paper-regime launch is cut into 64 parts of which the first --parts run
+PAPER_PARTS = int(os.environ.get("ARKCOS_AUDIT_PAPER_PARTS", "64"))   # the paper-regime launch is cut into this many parts of which the first --parts run
 
 
 def workload(cfg, k):

@@ -47,6 +47,9 @@ def test_kernels_present_for_sm100_and_no_local_memory(sass):
     for key in ("k_generate_weights", "k_convolve_wideE", "k_convolve_wide_tc", "k_convolve_narrow", "k_rfft_rings", "k_spectral_apply", "k_spectral_weights"):
         ops = [opcode(l) for l in find(sass, key)]
         assert not any(o.startswith(("LDL", "STL")) for o in ops), f"{key} spills to local memory"
+        if key.startswith("k_convolve"):       # every shared-memory access (stages, run tables, the partial sums of the
+            # blocked summation) was resolved to the shared address space: no generic-address loads or stores
+            assert not any(o.startswith(("LD.", "ST.")) for o in ops), f"{key} has generic-address memory accesses"
 
 
 def test_hot_loops_are_unrolled_plain_ffma_with_cp_async_staging(sass):
