@@ -134,3 +134,39 @@ def test_gaussian_beam_split_scenario():
     t_gpu = 0.0232 * cuts[cand] + 2.428
     t_cpu = 160.0 * max(l_cut, 0) ** 2 * l_max / 4096.0 ** 3
     assert abs(t - max(t_gpu, t_cpu)) < 1e-12
+
+
+def test_split_search_consumes_a_b200_cost_curve_built_from_the_plans_work_counts():
+    """The cost curve the split optimiser consumes (Eq. 2.3), for this library's direct sum on B200.
+    NO measured B200 curve exists yet (GPU access closed): the curve here is a MODEL - the exact
+    kernel-pixel evaluation counts of the real plans of configs[4] (theta_cut = 5, 10, 20, 40 arcmin on 4096 x 8192)
+    divided by the FMA rate round 1 measured (58.4 % of 148 x 128 x 1.965e9 FMA/s, commit 2dde936).  It checks the
+    pipeline plan work -> quadratic fit -> arkcos_split_search, and that a direct sum is quadratic, not linear, in
+    theta_cut.  `bench.py --sweep` prints the same two fits from measured times."""
+    rate = 0.584 * 148 * 128 * 1.965e9
+    cuts, t = [], []
+    for w in wl.config(4):
+        with arkcos.Plan(w.n_theta, w.n_phi, np.ones(16), w.theta_cut, flags=arkcos.PLAN_HOST_ONLY) as plan:
+            cuts.append(w.theta_cut / wl.ARCMIN)
+            t.append(plan.work()[0] / rate)
+    cuts, t = np.array(cuts), np.array(t)
+    quad = np.linalg.lstsq(np.stack([cuts ** 2, np.ones_like(cuts)], 1), t, rcond=None)[0]
+    lin = np.linalg.lstsq(np.stack([cuts, np.ones_like(cuts)], 1), t, rcond=None)[0]
+    res_q = np.sqrt(np.mean((quad[0] * cuts ** 2 + quad[1] - t) ** 2))
+    res_l = np.sqrt(np.mean((lin[0] * cuts + lin[1] - t) ** 2))
+    assert quad[0] > 0 and res_q < 0.05 * t.max() and res_q < 0.2 * res_l        # the quadratic form fits, the linear does not
+    assert 2e-3 < quad[0] * 40.0 ** 2 + quad[1] < 2e-2                            # ~5 ms per map at 40 arcmin
+    # the Gaussian-beam scenario of the test above with this cost model in place of Eq. 2.3
+    l_max = 768
+    sig = math.radians(30.0 / 60.0) / math.sqrt(8.0 * math.log(2.0))
+    k = split.table_legendre(wl.gaussian_table(sig, 12 * sig, 32769), 12 * sig, l_max)
+    cand_cuts = np.array([20.0, 30.0, 45.0, 60.0, 90.0])
+    b = np.stack([split.table_legendre(wl.gaussian_table(sig, math.radians(c / 60.0), 16385), math.radians(c / 60.0), l_max) for c in cand_cuts])
+    b200 = dict(gpu_a2=float(quad[0]), gpu_a1=0.0, gpu_c=float(max(quad[1], 0.0)), cpu_full_s=160.0, cpu_l_ref=4096.0)
+    c_b, l_b, t_b, s_b = split.split_search(k, cand_cuts, b, 1e-5, compensate=True, alpha=5.0, cost=b200)
+    c_p, l_p, t_p, s_p = split.split_search(k, cand_cuts, b, 1e-5, compensate=True, alpha=5.0, cost=split.PAPER_COST)
+    assert c_b >= 0 and s_b <= 1e-5
+    t_gpu = b200["gpu_a2"] * cand_cuts[c_b] ** 2 + b200["gpu_c"]
+    assert abs(t_b - max(t_gpu, 160.0 * max(l_b, 0) ** 2 * l_max / 4096.0 ** 3)) < 1e-12
+    # a GPU half that costs milliseconds moves the optimum to the wider cut / the smaller l_cut, and the pair is faster
+    assert c_b >= c_p and l_b <= l_p and t_b < t_p
