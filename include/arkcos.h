@@ -103,6 +103,10 @@ arkcos_status arkcos_plan_create_biased(arkcos_plan **plan, int n_theta, int n_p
  * call rewrites each weight with the bit-identical value, and each call's own S2 precedes its own S3 on its
  * stream, so concurrent calls never observe a different value (cached plans do not write at all).
  * The current device must be the plan's device.
+ * The map must be finite: windows are padded to whole 2- / 4- / 16-tap steps with ZERO weights, so an Inf or NaN
+ * input pixel makes the outputs within theta_cut of it - and up to 15 pixels further along its ring - NaN
+ * (0 x Inf), where the definition would give NaN only inside theta_cut.  Results are deterministic: one owner per
+ * output, fixed summation order (blocks of <= ~1000 taps).
  * Errors: EINVAL (NULL / misaligned / overlapping pointers, wrong current device), EUNSUPPORTED (host-only
  * plan), ECUDA.
  */
