@@ -438,18 +438,24 @@ def sweep(args):
             key = w.name.split("_cut")[0] + ("" if path == "direct" else " [spectral path]")
             curve.setdefault(key, []).append((w.theta_cut / wl.ARCMIN, line["ms_per_step"] / res["n_maps"]))
     for key, pts in curve.items():
-        if len(pts) < 3:
-            continue
-        t = np.array([p[0] for p in pts]); ms = np.array([p[1] for p in pts])
-        quad = np.linalg.lstsq(np.stack([t ** 2, np.ones_like(t)], 1), ms, rcond=None)[0]
-        lin = np.linalg.lstsq(np.stack([t, np.ones_like(t)], 1), ms, rcond=None)[0]
-        print(json.dumps({"report": "cost_curve", "family": key, "theta_cut_arcmin": t.tolist(), "gpu_ms_per_map": ms.tolist(),
-                          "fit_quadratic_ms": {"a_per_arcmin2": quad[0], "c": quad[1],
-                                               "rms_resid": float(np.sqrt(np.mean((quad[0] * t ** 2 + quad[1] - ms) ** 2)))},
-                          "fit_linear_ms": {"a_per_arcmin": lin[0], "c": lin[1],
-                                            "rms_resid": float(np.sqrt(np.mean((lin[0] * t + lin[1] - ms) ** 2)))},
-                          "paper_eq_2_3": "t = 0.0232 s * theta_cut[arcmin] + 2.428 s (GTX 480, HEALPix nside 2048; context only)"}),
-              flush=True)
+        if len(pts) >= 3:
+            print(json.dumps(cost_curve_line(key, pts)), flush=True)
+
+
+def cost_curve_line(key, pts):
+    """Least-squares fits of GPU time per map against theta_cut [arcmin]: a*cut^2 + c (a direct sum) and the paper's
+    linear form a*cut + c (Eq. 2.3); the coefficients are what arkcos_split_search consumes
+    (include/arkcos_split.h: gpu_a2 / gpu_a1 / gpu_c, there in seconds)."""
+    t = np.array([p[0] for p in pts], dtype=np.float64); ms = np.array([p[1] for p in pts], dtype=np.float64)
+    quad = np.linalg.lstsq(np.stack([t ** 2, np.ones_like(t)], 1), ms, rcond=None)[0]
+    lin = np.linalg.lstsq(np.stack([t, np.ones_like(t)], 1), ms, rcond=None)[0]
+    return {"report": "cost_curve", "family": key, "theta_cut_arcmin": t.tolist(), "gpu_ms_per_map": ms.tolist(),
+            "fit_quadratic_ms": {"a_per_arcmin2": float(quad[0]), "c": float(quad[1]),
+                                 "rms_resid": float(np.sqrt(np.mean((quad[0] * t ** 2 + quad[1] - ms) ** 2)))},
+            "fit_linear_ms": {"a_per_arcmin": float(lin[0]), "c": float(lin[1]),
+                              "rms_resid": float(np.sqrt(np.mean((lin[0] * t + lin[1] - ms) ** 2)))},
+            "split_cost_model_s": {"gpu_a2": float(quad[0]) * 1e-3, "gpu_a1": 0.0, "gpu_c": float(max(quad[1], 0.0)) * 1e-3},
+            "paper_eq_2_3": "t = 0.0232 s * theta_cut[arcmin] + 2.428 s (GTX 480, HEALPix nside 2048; context only)"}
 
 
 if __name__ == "__main__":

@@ -50,3 +50,17 @@ def test_other_bench_modes_run(args, expect):
         assert line[k] == v, (k, line.get(k))
     if "--impl" in args:
         assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["cpu_baseline"]["value"] == line["value"]
+
+
+def test_cost_curve_fits_of_the_sweep():
+    """bench.py --sweep's fit of GPU time against theta_cut (no device needed): a quadratic curve is recovered by the
+    quadratic form and not by the paper's linear form (Eq. 2.3), and the line carries the coefficients in
+    the units arkcos_split_search takes."""
+    sys.path.insert(0, ROOT)
+    import bench
+    cuts = [5.0, 10.0, 20.0, 40.0]
+    line = bench.cost_curve_line("cfg4", [(c, 0.05 + 3e-3 * c * c) for c in cuts])
+    q, l = line["fit_quadratic_ms"], line["fit_linear_ms"]
+    assert abs(q["a_per_arcmin2"] - 3e-3) < 1e-12 and abs(q["c"] - 0.05) < 1e-9 and q["rms_resid"] < 1e-9 < l["rms_resid"]
+    assert abs(line["split_cost_model_s"]["gpu_a2"] - 3e-6) < 1e-15 and line["theta_cut_arcmin"] == cuts
+    json.dumps(line)
